@@ -1,0 +1,146 @@
+/*
+ * mcb.h -- C ABI of libmcb: the bosonic Fock-space hot path of Andriati & Gammal, "Hashing algorithms,
+ * optimized mappings and massive parallelization of multiconfigurational methods for bosons"
+ * (arXiv 2005.13679; citations "PAPER.md:N" are lines of the paper text), hand-written for NVIDIA B200
+ * (sm_100a).  One GPU, one process.  No CPU fallback: every entry point that computes runs CUDA kernels.
+ *
+ * The problem (Eq. 7, 12, 13): N bosons in M orbitals ("IPS") span
+ *     nc = N_c(N, M) = binom(N+M-1, M-1)                                     (Eq. 7)
+ * configurations |n_0 .. n_{M-1}>, sum n_j = N, enumerated by the combinatorial perfect hash of Sec. III
+ * (Eq. 14; Algorithm 1; Algorithm 2), 0-based.
+ * Given one- and two-body matrix elements T (M x M) and V (M^4) and a complex vector C of length nc,
+ *     HC_g = sum_b <n^g| H |n^b> C_b,
+ *     H = sum_{k,l} T[k][l] a+_k a_l + 1/2 sum_{k,s,q,l} V[k][s][q][l] a+_k a+_s a_q a_l     (Eq. 3, 4, 12, 13)
+ * is computed without ever storing H.
+ *
+ * Conventions
+ *   - every function returning int returns MCB_OK (0) or a negative MCB_E* code; nothing throws or aborts.
+ *   - "d_" arguments are DEVICE pointers, "h_"/unprefixed array arguments are HOST pointers.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  All device work is
+ *     enqueued on it and is asynchronous unless stated otherwise.
+ *   - the library never allocates or frees caller-visible device memory.  The only device memory it owns
+ *     is a few hundred KB of constants per mcb_space (binomial / sqrt tables, packed T,V), allocated in
+ *     mcb_space_create and released in mcb_space_destroy.  Hashing table, jump maps and apply workspace
+ *     live in caller-provided device buffers (e.g. torch tensors) which must stay alive, unmodified,
+ *     for as long as the space uses them.
+ *   - complex numbers are interleaved (re, im) doubles == C99 double complex == torch.complex128.
+ *   - a mcb_space is not thread-safe: calls on one space must be serialised by the caller, and calls on
+ *     one space must all use the same stream or be ordered by the caller (T, V are staged per call in a
+ *     device buffer owned by the space).
+ */
+#ifndef MCB_H
+#define MCB_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MCB_OK            0
+#define MCB_EINVAL       -1   /* null pointer, N < 1, M < 1, aliasing, bad enum value                      */
+#define MCB_ERANGE       -2   /* nc >= 2^31 - 1 (indices are int32, PAPER.md:268-273 reading A14), M too large */
+#define MCB_ENOMEM       -3   /* caller buffer too small / host or device constant allocation failed        */
+#define MCB_ECUDA        -4   /* a CUDA runtime call failed; see mcb_last_cuda_error()                       */
+#define MCB_ENOTREADY    -5   /* a structure the call needs (hashing table, map) has not been built          */
+#define MCB_EUNSUPPORTED -6   /* M > MCB_MAX_M_APPLY for hc_apply, or mode not available for this space       */
+
+#define MCB_MAX_M        32   /* hashing and map kernels                                                      */
+#define MCB_MAX_M_APPLY  12   /* hc_apply: packed V (P x P complex, P = M(M+1)/2) must fit on chip            */
+
+/* structures that live in caller-provided device memory (mcb_structure_bytes / mcb_build_structure) */
+#define MCB_FOCK_TABLE    0   /* "hashing table" of all occupation vectors, for the N- and
+                                 (N-2)-particle spaces; needed by every hc_apply mode                         */
+#define MCB_MAP1          1   /* single-jump map                                           */
+#define MCB_MAP2          2   /* double-jump map, dense [pair(k<=s)][pair(q<=l)][b] layout  */
+
+/* hc_apply modes */
+#define MCB_AUTO          0   /* MCB_GEMM if N >= 2, else MCB_REHASH                                           */
+#define MCB_MAPS          1   /* per-output gather through the stored Map1 + Map2 (the paper's fastest CPU/GPU
+                                 variant); needs FOCK_TABLE, MAP1, MAP2                      */
+#define MCB_REHASH        2   /* per-output gather, target indices recomputed on the fly from the hashing table
+                                 ("hashing table + algorithm 1" variant); needs FOCK_TABLE       */
+#define MCB_GEMM          3   /* on-the-fly rehashing, two-body term factored through the (N-2)-particle space:
+                                 W = Vpacked . (F * C[jump]) as an FP64 tensor-core contraction, then a gather;
+                                 T folded into V via sum_s a+_s a_s = N.  needs FOCK_TABLE and a workspace     */
+
+typedef struct mcb_space mcb_space;          /* opaque */
+typedef struct { double re, im; } mcb_c128;
+
+/* ---- space ------------------------------------------------------------------------------------------ */
+
+/* Create the configuration space of N >= 1 bosons in 1 <= M <= MCB_MAX_M orbitals on the CURRENT CUDA
+ * device.  Builds the binomial table N_c(n,m) (Eq. 7, 14) on the host and uploads small device constants.
+ * MCB_ERANGE if nc >= 2^31 - 1.  *out is set to NULL on failure. */
+int  mcb_space_create(int N, int M, mcb_space** out);
+void mcb_space_destroy(mcb_space* sp);                        /* NULL is allowed */
+
+long long mcb_nc(const mcb_space* sp);                        /* N_c(N, M); -1 if sp is NULL */
+long long mcb_nc_removed(const mcb_space* sp, int r);         /* N_c(N - r, M), r = 0, 1, 2 (0 if N - r < 0) */
+/* host_out: (N+1) x (M+1) long long, row-major [n][m]: N_c(n,m) = binom(n+m-1, m-1), N_c(n,0) = 0. */
+int  mcb_binom_table(const mcb_space* sp, long long* host_out);
+
+/* ---- batched hashing (Algorithms 1 and 2) ----------------------------------------------------------- */
+
+/* Algorithm 2 for a batch: d_idx int32[batch] -> d_occ int32[batch][M] (row-major).  An index outside
+ * [0, nc) yields a row of -1.  batch == 0 is a no-op. */
+int  mcb_unrank(const mcb_space* sp, const int* d_idx, long long batch, int* d_occ, void* stream);
+/* Algorithm 1 for a batch: d_occ int32[batch][M] -> d_idx int32[batch].  A row with a negative entry or
+ * with sum != N yields -1. */
+int  mcb_rank(const mcb_space* sp, const int* d_occ, long long batch, int* d_idx, void* stream);
+
+/* ---- hashing table and jump maps (built once per space) ---------------------------- */
+
+/* Bytes the structure needs; < 0 is an MCB_E* code. */
+long long mcb_structure_bytes(const mcb_space* sp, int which);
+/* Build structure `which` into d_buf (256-byte aligned, at least mcb_structure_bytes) and attach it to the
+ * space.  Rebuilding replaces the attachment.  The buffer is owned by the caller. */
+int  mcb_build_structure(mcb_space* sp, int which, void* d_buf, long long bytes, void* stream);
+/* Detach (the caller is about to free the buffer). */
+int  mcb_detach_structure(mcb_space* sp, int which);
+
+/* Logical views for parity tests (synchronous: they synchronise `the build stream` via cudaDeviceSynchronize
+ * and copy to host):
+ *   fock: host_out int32[count][M]          occupation vector of configurations b0 .. b0+count-1 of the
+ *                                           (N - removed)-particle space, removed in {0, 2}
+ *   map1: host_out int32[count][M][M]       Map1[b][k][l] = index of n^(b) - e_k + e_l, -1 if n_k = 0;
+ *                                           the diagonal k == l is b itself when n_k >= 1
+ *   map2: host_out int32[count][P][P]       Map2[b][(k<=s)][(q<=l)] = index of n^(b) - e_k - e_s + e_q + e_l,
+ *                                           -1 if the removal is not allowed; pairs ordered (0,0),(0,1),..,
+ *                                           (0,M-1),(1,1),..,(M-1,M-1); P = M(M+1)/2 */
+int  mcb_fock_export(const mcb_space* sp, int removed, long long b0, long long count, int* host_out);
+int  mcb_map1_export(const mcb_space* sp, long long b0, long long count, int* host_out);
+int  mcb_map2_export(const mcb_space* sp, long long b0, long long count, int* host_out);
+
+/* ---- H.C (Eq. 12) ------------------------------------------------------------------------------------- */
+
+/* Device workspace hc_apply needs in `mode` (0 for MCB_MAPS / MCB_REHASH); < 0 is an MCB_E* code. */
+long long mcb_apply_workspace_bytes(const mcb_space* sp, int mode);
+
+/* d_HC = H . d_C.
+ *   T: host, M*M complex, T[k*M + l] multiplies a+_k a_l (Eq. 3).
+ *   V: host, M^4 complex, V[((k*M+s)*M+q)*M+l] multiplies 1/2 a+_k a+_s a_q a_l (Eq. 4, 13).  ANY tensor
+ *      is accepted; only its part symmetric under k<->s and q<->l contributes for bosons, and the library
+ *      packs exactly that part.  T, V are read before the call returns.
+ *   d_C, d_HC: device, nc complex each, 16-byte aligned, must not overlap.
+ *   d_workspace: device, mcb_apply_workspace_bytes(sp, mode) bytes, 256-byte aligned (may be NULL if 0).
+ * Asynchronous on `stream`.  M must be <= MCB_MAX_M_APPLY. */
+int  mcb_hc_apply(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
+                  const mcb_c128* d_C, mcb_c128* d_HC, int mode, void* d_workspace, void* stream);
+
+/* Same with HOST vectors: copies h_C (nc complex) to d_C_scratch, applies, copies the result from
+ * d_HC_scratch to h_HC, and synchronises the stream before returning.  h_C / h_HC should be pinned for
+ * full PCIe bandwidth but need not be. */
+int  mcb_hc_apply_host(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
+                       const mcb_c128* h_C, mcb_c128* h_HC, int mode,
+                       mcb_c128* d_C_scratch, mcb_c128* d_HC_scratch, void* d_workspace, void* stream);
+
+/* Number of kernels the last mcb_hc_apply on this space launched (for launch accounting). */
+int  mcb_last_apply_launches(const mcb_space* sp);
+
+/* ---- errors ------------------------------------------------------------------------------------------- */
+const char* mcb_strerror(int status);
+int         mcb_last_cuda_error(void);       /* cudaError_t of the last failing CUDA call in this thread */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MCB_H */

@@ -1,0 +1,248 @@
+"""paper_2005_13679_b200 -- thin Python binding of libmcb (include/mcb.h).
+
+Argument marshalling only: every step of the hot path (Algorithm 1 / 2 batches, hashing table, jump maps,
+H.C) runs in the hand-written sm_100a kernels behind the C ABI.  PyTorch is used for device memory and
+streams.  There is no CPU fallback: importing works without a GPU (so the symbol table can be checked), but
+any compute call without the built library or without a CUDA device raises.
+
+Names follow include/mcb.h: Space.unrank / rank / build_structure / hc_apply / hc_apply_host ...
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libmcb.so")
+
+OK, EINVAL, ERANGE, ENOMEM, ECUDA, ENOTREADY, EUNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
+FOCK_TABLE, MAP1, MAP2 = 0, 1, 2
+AUTO, MAPS, REHASH, GEMM = 0, 1, 2, 3
+MAX_M, MAX_M_APPLY = 32, 12
+
+EXPORTS = (
+    "mcb_space_create", "mcb_space_destroy", "mcb_nc", "mcb_nc_removed", "mcb_binom_table",
+    "mcb_unrank", "mcb_rank", "mcb_structure_bytes", "mcb_build_structure", "mcb_detach_structure",
+    "mcb_fock_export", "mcb_map1_export", "mcb_map2_export", "mcb_apply_workspace_bytes",
+    "mcb_hc_apply", "mcb_hc_apply_host", "mcb_last_apply_launches", "mcb_strerror", "mcb_last_cuda_error",
+)
+
+_lib = None
+
+
+class McbError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        msg = lib().mcb_strerror(status).decode()
+        if status == ECUDA:
+            msg += f" [cudaError {lib().mcb_last_cuda_error()}]"
+        super().__init__(f"{where}: {msg} ({status})")
+
+
+def lib():
+    """Load libmcb.so (built in-tree by paper_2005_13679_b200.build); fails loudly if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2005_13679_b200.build` "
+                              "(there is no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        vp, ll, i = ctypes.c_void_p, ctypes.c_longlong, ctypes.c_int
+        L.mcb_space_create.argtypes = [i, i, ctypes.POINTER(vp)]
+        L.mcb_space_destroy.argtypes = [vp]
+        L.mcb_space_destroy.restype = None
+        L.mcb_nc.argtypes = [vp]; L.mcb_nc.restype = ll
+        L.mcb_nc_removed.argtypes = [vp, i]; L.mcb_nc_removed.restype = ll
+        L.mcb_binom_table.argtypes = [vp, vp]
+        L.mcb_unrank.argtypes = [vp, vp, ll, vp, vp]
+        L.mcb_rank.argtypes = [vp, vp, ll, vp, vp]
+        L.mcb_structure_bytes.argtypes = [vp, i]; L.mcb_structure_bytes.restype = ll
+        L.mcb_build_structure.argtypes = [vp, i, vp, ll, vp]
+        L.mcb_detach_structure.argtypes = [vp, i]
+        L.mcb_fock_export.argtypes = [vp, i, ll, ll, vp]
+        L.mcb_map1_export.argtypes = [vp, ll, ll, vp]
+        L.mcb_map2_export.argtypes = [vp, ll, ll, vp]
+        L.mcb_apply_workspace_bytes.argtypes = [vp, i]; L.mcb_apply_workspace_bytes.restype = ll
+        L.mcb_hc_apply.argtypes = [vp, vp, vp, vp, vp, i, vp, vp]
+        L.mcb_hc_apply_host.argtypes = [vp, vp, vp, vp, vp, i, vp, vp, vp, vp]
+        L.mcb_last_apply_launches.argtypes = [vp]
+        L.mcb_strerror.argtypes = [i]; L.mcb_strerror.restype = ctypes.c_char_p
+        L.mcb_last_cuda_error.argtypes = []
+        _lib = L
+    return _lib
+
+
+def _check(status: int, where: str):
+    if status != OK:
+        raise McbError(status, where)
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_2005_13679_b200 needs a CUDA device (no CPU fallback)")
+    return torch
+
+
+def _stream_ptr(stream) -> int:
+    torch = _torch()
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return int(s.cuda_stream)
+
+
+def _host_c128(a, shape) -> np.ndarray:
+    a = np.ascontiguousarray(a, dtype=np.complex128)
+    if a.size != int(np.prod(shape)):
+        raise ValueError(f"expected {shape} complex values, got {a.shape}")
+    return a
+
+
+class Space:
+    """N bosons in M orbitals (include/mcb.h mcb_space).  Owns the torch buffers of the structures it builds."""
+
+    def __init__(self, N: int, M: int, device=None):
+        torch = _torch()
+        self.N, self.M = int(N), int(M)
+        self.P = self.M * (self.M + 1) // 2
+        self.device = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
+        self._h = ctypes.c_void_p()
+        with torch.cuda.device(self.device):
+            _check(lib().mcb_space_create(self.N, self.M, ctypes.byref(self._h)), "mcb_space_create")
+        self.nc = int(lib().mcb_nc(self._h))
+        self.nc2 = int(lib().mcb_nc_removed(self._h, 2))
+        self._buffers = {}
+        self._workspace = {}
+
+    # -- lifetime -----------------------------------------------------------------------------------------
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h:
+            _torch().cuda.synchronize(self.device)
+            lib().mcb_space_destroy(self._h)
+            self._h = ctypes.c_void_p()
+            self._buffers.clear()
+            self._workspace.clear()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- tables -------------------------------------------------------------------------------------------
+    def binom_table(self) -> np.ndarray:
+        out = np.zeros((self.N + 1, self.M + 1), dtype=np.int64)
+        _check(lib().mcb_binom_table(self._h, out.ctypes.data), "mcb_binom_table")
+        return out
+
+    def nc_removed(self, r: int) -> int:
+        return int(lib().mcb_nc_removed(self._h, r))
+
+    # -- batched hashing ------------------------------------------------------------------------------------
+    def unrank(self, idx, stream=None):
+        """int32 device tensor [batch] -> int32 device tensor [batch, M] (Algorithm 2)."""
+        torch = _torch()
+        idx = idx.to(device=self.device, dtype=torch.int32).contiguous()
+        occ = torch.empty((idx.numel(), self.M), dtype=torch.int32, device=self.device)
+        _check(lib().mcb_unrank(self._h, idx.data_ptr(), idx.numel(), occ.data_ptr(), _stream_ptr(stream)), "mcb_unrank")
+        return occ
+
+    def rank(self, occ, stream=None):
+        """int32 device tensor [batch, M] -> int32 device tensor [batch] (Algorithm 1)."""
+        torch = _torch()
+        occ = occ.to(device=self.device, dtype=torch.int32).contiguous().view(-1, self.M)
+        idx = torch.empty((occ.shape[0],), dtype=torch.int32, device=self.device)
+        _check(lib().mcb_rank(self._h, occ.data_ptr(), occ.shape[0], idx.data_ptr(), _stream_ptr(stream)), "mcb_rank")
+        return idx
+
+    # -- structures ---------------------------------------------------------------------------------------
+    def structure_bytes(self, which: int) -> int:
+        n = int(lib().mcb_structure_bytes(self._h, which))
+        if n < 0:
+            raise McbError(n, "mcb_structure_bytes")
+        return n
+
+    def build_structure(self, which: int, stream=None):
+        """Allocate a torch buffer of mcb_structure_bytes and build the structure into it."""
+        torch = _torch()
+        nbytes = self.structure_bytes(which)
+        buf = torch.empty(max(nbytes, 256), dtype=torch.uint8, device=self.device)
+        assert buf.data_ptr() % 256 == 0
+        _check(lib().mcb_build_structure(self._h, which, buf.data_ptr(), nbytes, _stream_ptr(stream)), "mcb_build_structure")
+        self._buffers[which] = buf
+        return buf
+
+    def drop_structure(self, which: int):
+        _torch().cuda.synchronize(self.device)
+        _check(lib().mcb_detach_structure(self._h, which), "mcb_detach_structure")
+        self._buffers.pop(which, None)
+
+    def fock_export(self, b0: int, count: int, removed: int = 0) -> np.ndarray:
+        out = np.empty((count, self.M), dtype=np.int32)
+        _check(lib().mcb_fock_export(self._h, removed, b0, count, out.ctypes.data), "mcb_fock_export")
+        return out
+
+    def map1_export(self, b0: int, count: int) -> np.ndarray:
+        out = np.empty((count, self.M, self.M), dtype=np.int32)
+        _check(lib().mcb_map1_export(self._h, b0, count, out.ctypes.data), "mcb_map1_export")
+        return out
+
+    def map2_export(self, b0: int, count: int) -> np.ndarray:
+        out = np.empty((count, self.P, self.P), dtype=np.int32)
+        _check(lib().mcb_map2_export(self._h, b0, count, out.ctypes.data), "mcb_map2_export")
+        return out
+
+    # -- H.C ----------------------------------------------------------------------------------------------
+    def apply_workspace_bytes(self, mode: int = AUTO) -> int:
+        n = int(lib().mcb_apply_workspace_bytes(self._h, mode))
+        if n < 0:
+            raise McbError(n, "mcb_apply_workspace_bytes")
+        return n
+
+    def _ws(self, mode: int):
+        torch = _torch()
+        n = self.apply_workspace_bytes(mode)
+        if n == 0:
+            return 0
+        w = self._workspace.get("ws")
+        if w is None or w.numel() < n:
+            w = torch.empty(n, dtype=torch.uint8, device=self.device)
+            self._workspace["ws"] = w
+        return w.data_ptr()
+
+    def hc_apply(self, T, V, C, out=None, mode: int = AUTO, stream=None):
+        """HC = H.C for a complex128 device tensor C [nc]; T [M,M], V [M,M,M,M] host arrays."""
+        torch = _torch()
+        T = _host_c128(T, (self.M, self.M))
+        V = _host_c128(V, (self.M,) * 4)
+        if C.dtype != torch.complex128 or not C.is_cuda or not C.is_contiguous() or C.numel() != self.nc:
+            raise ValueError("C must be a contiguous complex128 CUDA tensor of length nc")
+        if out is None:
+            out = torch.empty_like(C)
+        _check(lib().mcb_hc_apply(self._h, T.ctypes.data, V.ctypes.data, C.data_ptr(), out.data_ptr(), mode,
+                                  self._ws(mode), _stream_ptr(stream)), "mcb_hc_apply")
+        return out
+
+    def hc_apply_host(self, T, V, C_host, out_host=None, mode: int = AUTO, stream=None):
+        """Same through host memory: C_host / out_host are complex128 CPU tensors (pinned for full PCIe speed)
+        or numpy arrays.  Copies H2D, applies, copies D2H, synchronises."""
+        torch = _torch()
+        T = _host_c128(T, (self.M, self.M))
+        V = _host_c128(V, (self.M,) * 4)
+        if isinstance(C_host, np.ndarray):
+            C_host = torch.from_numpy(np.ascontiguousarray(C_host, dtype=np.complex128))
+        if C_host.numel() != self.nc or C_host.dtype != torch.complex128 or C_host.is_cuda:
+            raise ValueError("C_host must be a complex128 CPU tensor of length nc")
+        if out_host is None:
+            out_host = torch.empty_like(C_host)
+        for name in ("dC", "dHC"):
+            if name not in self._workspace:
+                self._workspace[name] = torch.empty(self.nc, dtype=torch.complex128, device=self.device)
+        _check(lib().mcb_hc_apply_host(self._h, T.ctypes.data, V.ctypes.data, C_host.data_ptr(), out_host.data_ptr(),
+                                       mode, self._workspace["dC"].data_ptr(), self._workspace["dHC"].data_ptr(),
+                                       self._ws(mode), _stream_ptr(stream)), "mcb_hc_apply_host")
+        return out_host
+
+    def last_apply_launches(self) -> int:
+        return int(lib().mcb_last_apply_launches(self._h))

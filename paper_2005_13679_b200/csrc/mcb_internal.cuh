@@ -1,0 +1,61 @@
+// mcb_internal.cuh -- shared declarations of libmcb (the CUDA product path; nothing here is used by oracle/).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "mcb.h"
+
+// ---- device-side view of the small per-space constants -------------------------------------------------
+// G[j][s] = binom(s + j, j + 1), j = 0..M-2, s = 0..N: the number of configurations that precede, in the
+// order of Eq. (14), every configuration whose prefix sum S_j = n_0 + .. + n_j equals s
+// *because of digit j alone*.  With it Algorithm 1's index collapses (hockey stick) to
+//     index(n) = nc - 1 - sum_{j=0}^{M-2} G[j][S_j]
+// which is what every kernel uses: O(M) look-ups instead of Algorithm 1's O(N) additions.
+struct McbDev {
+    int N, M;
+    int nc, nc1, nc2;          // N_c(N,M), N_c(N-1,M), N_c(N-2,M)
+    int ldg;                   // row stride of G (= N + 1)
+    const int* G;              // [(M-1)][ldg]   (M == 1: no rows)
+    const double* sq;          // sq[j]  = sqrt(j),          j = 0..N+2
+    const double* sq2;         // sq2[j] = sqrt(j (j - 1)),  j = 0..N+2   (sq2[0] = sq2[1] = 0)
+};
+
+struct McbFockView {           // hashing table, SoA uint16: occ[j][b], row stride ld
+    const uint16_t* occ;       // N-particle space
+    long long ld;
+    const uint16_t* occ2;      // (N-2)-particle space (NULL if N < 2)
+    long long ld2;
+};
+
+struct mcb_space {
+    int N, M, P;
+    int device;
+    long long nc, nc1, nc2;
+    long long* h_binom;        // (N+1) x (M+1), N_c(n, m)
+    void* d_consts;            // one allocation holding G, sq, sq2
+    McbDev dev;
+    // attached caller-owned structures
+    void* d_fock; long long fock_bytes; McbFockView fock;
+    int* d_map1;  long long map1_ld;     // [k][l][b], row stride map1_ld
+    int* d_map2;  long long map2_ld;     // [ks][ql][b]
+    // per-apply staging of packed T, V (device, owned)
+    void* d_coef; size_t coef_bytes;
+    void* h_coef;              // host scratch for packing
+    int last_launches;
+};
+
+static inline long long mcb_round_up(long long x, long long a) { return (x + a - 1) / a * a; }
+
+// error plumbing (mcb_space.cu)
+int mcb_set_cuda_error(cudaError_t e);
+#define MCB_CUDA(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return mcb_set_cuda_error(e__); } while (0)
+#define MCB_CHECK_LAUNCH() MCB_CUDA(cudaGetLastError())
+
+// ---- pair enumeration (k <= s), order (0,0),(0,1),..,(0,M-1),(1,1),..  (include/mcb.h) ------------------
+__host__ __device__ constexpr int mcb_pair_index(int M, int k, int s) { return k * M - k * (k - 1) / 2 + (s - k); }
+
+// implemented per translation unit
+int mcb_launch_unrank(const mcb_space* sp, const int* d_idx, long long batch, int* d_occ, cudaStream_t st);
+int mcb_launch_rank(const mcb_space* sp, const int* d_occ, long long batch, int* d_idx, cudaStream_t st);
+int mcb_launch_fock_table(const mcb_space* sp, int removed, uint16_t* d_out, long long ld, cudaStream_t st);
+int mcb_launch_map1(const mcb_space* sp, int* d_out, long long ld, cudaStream_t st);
+int mcb_launch_map2(const mcb_space* sp, int* d_out, long long ld, cudaStream_t st);

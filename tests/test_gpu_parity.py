@@ -1,0 +1,112 @@
+"""GPU parity: libmcb (CUDA, through the C ABI binding) vs the CPU oracle on the same seeded inputs.
+
+Integer work (hashing, hashing table, jump maps) must be bit-exact.  HC must satisfy
+    max_i |HC_gpu - HC_ref|_i <= 1e-12 * max(|T|_max, |V|_max) * ||C||_1        (BASELINE.json north_star; A19, A20).
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+import workloads
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def mcb():
+    import paper_2005_13679_b200 as m
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    m.lib()          # fails loudly if the CUDA library was not built
+    return m
+
+
+def tol(T, V, C):
+    return 1e-12 * max(np.abs(T).max(), np.abs(V).max()) * np.abs(C).sum()
+
+
+SMALL = [(1, 1), (1, 4), (4, 1), (2, 2), (3, 3), (2, 4), (10, 5), (6, 4), (5, 7), (7, 6), (40, 3), (3, 9), (4, 12), (2, 12),
+         (300, 2), (5, 10), (4, 11), (6, 8)]
+
+
+@pytest.mark.parametrize("N,M", SMALL + [(3, 20), (2, 32)])
+def test_unrank_rank_full_space(mcb, N, M):
+    sp = mcb.Space(N, M)
+    nc = math.comb(N + M - 1, M - 1)
+    assert sp.nc == nc
+    assert (sp.binom_table() == oracle.binom_table(N, M)).all()
+    idx = torch.arange(nc, dtype=torch.int32, device="cuda")
+    occ = sp.unrank(idx)
+    ref = oracle.unrank(N, M, np.arange(nc))
+    assert (occ.cpu().numpy() == ref).all()
+    back = sp.rank(occ)
+    assert (back.cpu().numpy() == np.arange(nc)).all()
+    sp.close()
+
+
+def test_hash_error_rows(mcb):
+    sp = mcb.Space(6, 4)
+    idx = torch.tensor([-1, 0, sp.nc - 1, sp.nc, 2 ** 31 - 1], dtype=torch.int32, device="cuda")
+    occ = sp.unrank(idx).cpu().numpy()
+    assert (occ[[0, 3, 4]] == -1).all() and occ[1].tolist() == [6, 0, 0, 0] and occ[2].tolist() == [0, 0, 0, 6]
+    bad = torch.tensor([[6, 0, 0, 0], [5, 0, 0, 0], [7, -1, 0, 0], [3, 2, 1, 0], [0, 0, 0, 7]], dtype=torch.int32, device="cuda")
+    got = sp.rank(bad).cpu().numpy()
+    assert got[0] == 0 and got[1] == -1 and got[2] == -1 and got[4] == -1
+    assert got[3] == oracle.rank(6, 4, np.array([[3, 2, 1, 0]]))[0]
+    assert sp.unrank(torch.empty(0, dtype=torch.int32, device="cuda")).shape == (0, 4)
+    sp.close()
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4])
+def test_hash_batches_on_full_size_configs(mcb, cfg):
+    c = workloads.CONFIGS[cfg]
+    sp = mcb.Space(c.N, c.M)
+    assert sp.nc == c.nc
+    idx = workloads.index_batch(c.nc, 1 << 20, workloads.seed_for(cfg, 7))
+    idx[:4] = [0, 1, c.nc - 2, c.nc - 1]
+    occ = sp.unrank(torch.from_numpy(idx).cuda())
+    sample = np.concatenate([np.arange(4), np.arange(4, idx.size, 997)])
+    assert (occ.cpu().numpy()[sample] == oracle.unrank(c.N, c.M, idx[sample])).all()
+    assert (occ.sum(dim=1) == c.N).all() and (occ >= 0).all()
+    assert (sp.rank(occ).cpu().numpy() == idx).all()            # round trip on all 2^20
+    sp.close()
+
+
+@pytest.mark.parametrize("N,M", SMALL)
+def test_structures_small(mcb, N, M):
+    sp = mcb.Space(N, M)
+    nc = sp.nc
+    sp.build_structure(mcb.FOCK_TABLE)
+    assert (sp.fock_export(0, nc) == oracle.unrank(N, M, np.arange(nc))).all()
+    if N >= 2:
+        nc2 = sp.nc2
+        assert nc2 == math.comb(N - 2 + M - 1, M - 1)
+        assert (sp.fock_export(0, nc2, removed=2) == oracle.unrank(N - 2, M, np.arange(nc2))).all()
+    sp.build_structure(mcb.MAP1)
+    assert (sp.map1_export(0, nc) == oracle.map1(N, M, 0, nc)).all()
+    if M <= 8:
+        sp.build_structure(mcb.MAP2)
+        assert (sp.map2_export(0, nc) == oracle.map2(N, M, 0, nc)).all()
+    sp.close()
+
+
+@pytest.mark.parametrize("N,M", SMALL)
+@pytest.mark.parametrize("mode", ["REHASH", "MAPS", "GEMM"])
+def test_hc_apply_small(mcb, N, M, mode):
+    if mode == "MAPS" and M > 8:
+        pytest.skip("Map2 not built for large M in the small-case sweep")
+    sp = mcb.Space(N, M)
+    nc = sp.nc
+    T, V, C = workloads.make_small_inputs(N, M, nc, seed=1000 + 17 * N + M, general_V=(N + M) % 2 == 0)
+    ref, _ = oracle.hc_apply(N, M, T, V, C)
+    sp.build_structure(mcb.FOCK_TABLE)
+    if mode == "MAPS":
+        sp.build_structure(mcb.MAP1)
+        sp.build_structure(mcb.MAP2)
+    got = sp.hc_apply(T, V, torch.from_numpy(C).cuda(), mode=getattr(mcb, mode)).cpu().numpy()
+    err = np.abs(got - ref).max()
+    assert err <= tol(T, V, C), (err, tol(T, V, C))
+    sp.close()
