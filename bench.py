@@ -1,0 +1,417 @@
+#!/usr/bin/env python
+"""bench.py -- H.C throughput of libmcb on B200, with the oracle timed beside it.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--cfg 0..4] [--mode auto|gemm|rehash|maps] [--impl reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P \
+        bench.py --gpus N --steps K --warmup W
+
+A "step" is one pass of the whole hot path's steady state over one coefficient vector: one
+`hc_apply(T, V, C) -> HC` (Eq. 12) through the C ABI (include/mcb.h), with the hashing table
+(and the jump maps in MAPS mode) already built on the device -- they are built once per space
+(PAPER.md:178-224); their build times are reported under "setup".  T and V are packed and uploaded inside
+every step (they change every step in the paper's motivating use).
+
+Headline workload = BASELINE.json configs[2] (N=400, M=4: the largest nc, which is what `metric` is quoted
+on).  `value` = configurations/s = nc * applications/s, whole job (all ranks; the path does not shard by
+north_star, so N>1 runs N independent replicas = weak scaling, no data-path collective).
+
+Cold-cache rule: inputs are larger than L2 -- the step rotates through R distinct C vectors and R distinct HC
+buffers whose total size (>= 3 * 2 * 16 * nc bytes) exceeds the 126 MB L2 several times over.
+
+One JSON line is printed by rank 0.  `--impl reference` times the CPU oracle (oracle/, as it stands) on the
+host cores on a bounded row sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import workloads  # noqa: E402
+
+METRIC = "hc_apply_configurations_per_s"
+UNIT = "configs/s"
+FP64_FMA_PER_CLK_PER_SM = 64          # B200 SM = 4 sub-partitions x 16 FP64 lanes
+N_SM = 148
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return {"hbm_gbs": float(d["hbm_gbs"]), "sm_max_mhz": float(d.get("sm_max_mhz", 1965.0)), "source": "measured"}
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback"}
+
+
+def fp64_peak_tflops(sm_mhz: float) -> float:
+    """Plain FP64 ALU peak: 148 SMs x 64 DFMA/clk x 2 flop x clock."""
+    return N_SM * FP64_FMA_PER_CLK_PER_SM * 2 * sm_mhz * 1e6 / 1e12
+
+
+def term_counts(N: int, M: int, nc: int, nc1: int, nc2: int):
+    """Algorithmic term counts per apply: one-body M^2*nc1, two-body (packed) P^2*nc2."""
+    P = M * (M + 1) // 2
+    return {"one_body_terms": M * M * nc1, "two_body_terms_packed": P * P * nc2, "P": P}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md clocks line)."""
+
+    def __init__(self, index: int, period_s: float = 0.05):
+        self.index, self.period = index, period_s
+        self.samples, self.reasons = [], set()
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._thr = None
+        self._nv = None
+
+    def start(self):
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nv = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self._nv = None
+        self._thr = threading.Thread(target=self._run, daemon=True)
+        self._thr.start()
+
+    def _run(self):
+        nv = self._nv
+        names = {}
+        if nv is not None:
+            for nm, key in (("nvmlClocksThrottleReasonHwSlowdown", "hw_slowdown"),
+                            ("nvmlClocksThrottleReasonHwThermalSlowdown", "hw_thermal_slowdown"),
+                            ("nvmlClocksThrottleReasonSwThermalSlowdown", "sw_thermal_slowdown"),
+                            ("nvmlClocksThrottleReasonSwPowerCap", "sw_power_cap"),
+                            ("nvmlClocksThrottleReasonHwPowerBrakeSlowdown", "hw_power_brake_slowdown")):
+                if hasattr(nv, nm):
+                    names[getattr(nv, nm)] = key
+        while not self._stop.is_set():
+            try:
+                if nv is not None:
+                    self.samples.append(float(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM)))
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self._h)
+                    for bit, key in names.items():
+                        if r & bit:
+                            self.reasons.add(key)
+                else:
+                    import subprocess
+                    out = subprocess.run(
+                        ["nvidia-smi", "-i", str(self.index),
+                         "--query-gpu=clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,"
+                         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+                         "clocks_event_reasons.sw_power_cap", "--format=csv,noheader,nounits"],
+                        capture_output=True, text=True, timeout=5).stdout.strip().split(",")
+                    self.samples.append(float(out[0]))
+                    self.max_mhz = float(out[1])
+                    for v, key in zip(out[2:], ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")):
+                        if v.strip().lower() == "active":
+                            self.reasons.add(key)
+            except Exception:
+                pass
+            self._stop.wait(self.period)
+
+    def stop(self):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join(timeout=5)
+        s = sorted(self.samples)
+        med = s[len(s) // 2] if s else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(s)}
+
+
+# ------------------------------------------------------------------------------------------------------------
+# CPU oracle legs
+# ------------------------------------------------------------------------------------------------------------
+def oracle_sample_rate(c, T, V, C, target_s: float, nthreads: int = 0):
+    """Time oracle.hc_apply on a bounded seeded row sample; returns (configs/s, threads, rows, seconds)."""
+    import oracle
+    probe = workloads.sample_rows(c.nc, 64, 1024, workloads.seed_for(c.cfg, 11))
+    t0 = time.perf_counter()
+    _, used = oracle.hc_apply(c.N, c.M, T, V, C, rows=probe, nthreads=nthreads)
+    dt = max(time.perf_counter() - t0, 1e-6)
+    rate = probe.size / dt
+    nrows = int(min(c.nc, max(probe.size, rate * target_s)))
+    if nrows >= c.nc:
+        rows = None
+        nrows = c.nc
+    else:
+        rows = workloads.sample_rows(c.nc, 1024, nrows, workloads.seed_for(c.cfg, 12))
+        nrows = rows.size
+    t0 = time.perf_counter()
+    _, used = oracle.hc_apply(c.N, c.M, T, V, C, rows=rows, nthreads=nthreads)
+    dt = time.perf_counter() - t0
+    return nrows / dt, used, nrows, dt
+
+
+def run_reference(args):
+    """--impl reference: the oracle as it stands, on the host cores; rank 0 only."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import oracle
+    oracle.build()
+    c, T, V, (C,) = workloads.make_inputs(args.cfg)
+    per_step_s = max(2.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
+    rates, rows_used, used = [], 0, 1
+    for i in range(args.warmup + args.steps):
+        r, used, nrows, dt = oracle_sample_rate(c, T, V, C, per_step_s)
+        if i >= args.warmup:
+            rates.append((nrows, dt))
+            rows_used = nrows
+    tot_rows = sum(n for n, _ in rates)
+    tot_s = sum(d for _, d in rates)
+    value = tot_rows / tot_s
+    sample = f"{rows_used} seeded rows of {c.nc} per step (rows of H.C are independent), all host threads"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * c.nc / value,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "complex128 (f64)",
+        "data": "synthetic (seeded, workloads.py)",
+        "config": config_dict(c, "oracle O6: ordered M^4 sums, literal Algorithm 1 per term"),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": used, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "note": "ms_per_step is the full-vector time extrapolated from the row sample",
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def config_dict(c, variant: str):
+    return {"workload": f"BASELINE.json configs[{c.cfg}] {c.name}: N={c.N} bosons, M={c.M} orbitals, nc={c.nc}, "
+                        f"{'Lieb-Liniger T,V (g=10, L=1)' if c.kind == 'll' else 'dense random Hermitian T, symmetric random V'}, "
+                        "random L2-normalised complex128 C",
+            "N": c.N, "M": c.M, "nc": c.nc, "variant": variant}
+
+
+# ------------------------------------------------------------------------------------------------------------
+# GPU arm
+# ------------------------------------------------------------------------------------------------------------
+MODES = {"auto": 0, "maps": 1, "rehash": 2, "gemm": 3}
+KERNELS = {1: ["k_hc_direct<M,maps>"], 2: ["k_hc_direct<M,rehash>"], 3: ["k_hc2_contract<M>", "k_hc2_reduce<M>"]}
+
+
+def time_mode(sp, mcb, torch, T, V, dCs, dHCs, mode, steps, warmup, barrier):
+    """Device time of `steps` applies (CUDA events on the launching stream), plus per-kernel times."""
+    R = len(dCs)
+    for i in range(warmup):
+        sp.hc_apply(T, V, dCs[i % R], out=dHCs[i % R], mode=mode)
+    torch.cuda.synchronize()
+    barrier()
+    sp.timing_enable(True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for i in range(steps):
+        sp.hc_apply(T, V, dCs[i % R], out=dHCs[i % R], mode=mode)
+    e1.record()
+    torch.cuda.synchronize()
+    barrier()
+    ms_total = e0.elapsed_time(e1)
+    kms, la = sp.timing_read(min(steps, 512))
+    sp.timing_enable(False)
+    launches = int(sp.last_apply_launches())
+    return ms_total, kms, launches
+
+
+def run_gpu(args):
+    import torch
+    import paper_2005_13679_b200 as mcb
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: libmcb has no CPU path")
+    mcb.lib()
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+
+    def max_over_ranks(x: float) -> float:
+        if dist is None:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    peaks = load_peaks()
+    R = 3
+    c, T, V, Cs = workloads.make_inputs(args.cfg, n_vectors=R)
+    sp = mcb.Space(c.N, c.M)
+    assert sp.nc == c.nc
+    nc, nc1, nc2 = sp.nc, sp.nc_removed(1), sp.nc_removed(2)
+    tc = term_counts(c.N, c.M, nc, nc1, nc2)
+
+    # ---- setup (once per space): hashing table, and the maps if the mode needs them ----
+    setup = {}
+    def timed_build(which, name):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(); sp.build_structure(which); b.record(); torch.cuda.synchronize()
+        setup[name + "_ms"] = a.elapsed_time(b)
+        setup[name + "_bytes"] = sp.structure_bytes(which)
+    timed_build(mcb.FOCK_TABLE, "fock_table")
+    timed_build(mcb.FOCK_TABLE, "fock_table")            # second build = warm timing
+    mode = MODES[args.mode]
+    if mode == 0:
+        mode = mcb.GEMM if c.N >= 2 else mcb.REHASH
+    map_bytes = 0
+    if mode == mcb.MAPS:
+        timed_build(mcb.MAP1, "map1")
+        timed_build(mcb.MAP2, "map2")
+        map_bytes = 4 * nc * (c.M * c.M - c.M) + 4 * nc * tc["P"] ** 2   # entries the kernel may read (upper bound)
+
+    dCs = [torch.from_numpy(C).cuda() for C in Cs]
+    dHCs = [torch.empty_like(d) for d in dCs]
+
+    # ---- device-resident timing ----
+    clocks = ClockSampler(local)
+    clocks.start()
+    ms_total, kms, launches = time_mode(sp, mcb, torch, T, V, dCs, dHCs, mode, args.steps, args.warmup, barrier)
+    clk = clocks.stop()
+    ms_total = max_over_ranks(ms_total)
+    ms_step = ms_total / args.steps
+    value = world * nc / (ms_step * 1e-3)
+
+    # ---- end to end through the public API with HOST buffers (pinned), H2D + D2H inside the timed region ----
+    hC = [torch.from_numpy(C).pin_memory() for C in Cs]
+    hHC = [torch.empty_like(h).pin_memory() for h in hC]
+    e2e_steps = max(3, min(args.steps, 10))
+    for i in range(2):
+        sp.hc_apply_host(T, V, hC[i % R], out_host=hHC[i % R], mode=mode)
+    torch.cuda.synchronize(); barrier()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for i in range(e2e_steps):
+        sp.hc_apply_host(T, V, hC[i % R], out_host=hHC[i % R], mode=mode)
+    b.record(); torch.cuda.synchronize(); barrier()
+    e2e_ms = max_over_ranks(a.elapsed_time(b)) / e2e_steps
+    e2e_value = world * nc / (e2e_ms * 1e-3)
+
+    # ---- roofline of the dominant kernel ----
+    kavg = kms.mean(axis=0) if len(kms) else np.zeros(3)
+    dom = int(np.argmax(kavg))
+    dom_ms = float(kavg[dom])
+    flops_step = 8.0 * (tc["one_body_terms"] + tc["two_body_terms_packed"])
+    unique_bytes = 32.0 * nc
+    fock_bytes = 2.0 * c.M * (nc + nc2)
+    alu_peak = fp64_peak_tflops(peaks["sm_max_mhz"])
+    if mode == mcb.MAPS:
+        alg_bytes = unique_bytes + map_bytes + 2.0 * c.M * nc
+        roofline = {"bound": "hbm", "kernel": KERNELS[mode][dom], "achieved": alg_bytes / (dom_ms * 1e-3) / 1e9,
+                    "peak": peaks["hbm_gbs"], "unit": "GB/s", "peak_source": peaks["source"], "traffic": None,
+                    "algorithmic_bytes_per_launch": alg_bytes}
+    else:
+        # contract kernel (GEMM mode) carries every two-body term + the folded one-body terms: 8 flop per packed term
+        kflops = 8.0 * tc["two_body_terms_packed"] if mode == mcb.GEMM else flops_step
+        roofline = {"bound": "alu", "kernel": KERNELS[mode][dom], "achieved": kflops / (dom_ms * 1e-3) / 1e12,
+                    "peak": alu_peak, "unit": "TFLOP/s",
+                    "peak_source": f"derived: 148 SM x 64 DFMA/clk x 2 x {peaks['sm_max_mhz']:.0f} MHz (DESIGN.md)",
+                    "traffic": None, "algorithmic_flops_per_launch": kflops}
+    roofline["frac"] = roofline["achieved"] / roofline["peak"]
+    roofline["kernel_ms"] = dom_ms
+    roofline["kernel_share_of_step"] = dom_ms / ms_step
+    hbm_unique = {"bytes_per_step": unique_bytes, "achieved_GBps": unique_bytes / (ms_step * 1e-3) / 1e9,
+                  "peak_GBps": peaks["hbm_gbs"], "frac": unique_bytes / (ms_step * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                  "note": "unique bytes of C and HC only (32*nc); the step is FP64-ALU bound, see DESIGN.md"}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "complex128 (f64)", "data": "synthetic (seeded, workloads.py)",
+        "config": dict(config_dict(c, {1: "MAPS", 2: "REHASH", 3: "GEMM"}[mode]),
+                       l2="inputs larger than L2: 3 rotating C and 3 rotating HC buffers, 16*nc bytes each",
+                       replicas="N>1 = independent replicas (path does not shard by north_star)"),
+        "applications_per_s": world / (ms_step * 1e-3),
+        "terms_per_s": world * (tc["one_body_terms"] + tc["two_body_terms_packed"]) / (ms_step * 1e-3),
+        "gflop_per_step": flops_step / 1e9,
+        "kernel_ms": {KERNELS[mode][i]: float(kavg[i]) for i in range(len(KERNELS[mode]))},
+        "gpu_launches": launches * args.steps,
+        "roofline": roofline, "hbm_unique": hbm_unique, "setup": setup, "clocks": clk,
+        "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms, "steps": e2e_steps,
+                "h2d_bytes_per_step": 16 * nc + 16 * (c.M ** 2 + c.M ** 4), "d2h_bytes_per_step": 16 * nc,
+                "api": "mcb_hc_apply_host (pinned host C and HC)"},
+    }
+
+    # ---- the other variants, short (map-memory vs recompute trade-off) ----
+    if args.variants and rank == 0 and world == 1:
+        var = {}
+        for name, m in (("REHASH", mcb.REHASH), ("GEMM", mcb.GEMM), ("MAPS", mcb.MAPS)):
+            if m == mode or (m == mcb.GEMM and c.N < 2):
+                continue
+            try:
+                if m == mcb.MAPS:
+                    need = sp.structure_bytes(mcb.MAP1) + sp.structure_bytes(mcb.MAP2)
+                    free, _ = torch.cuda.mem_get_info()
+                    if need > 0.8 * free:
+                        var[name] = {"skipped": f"maps need {need / 1e9:.1f} GB (PAPER.md:264: memory is the limit)"}
+                        continue
+                    sp.build_structure(mcb.MAP1); sp.build_structure(mcb.MAP2)
+                ms, km, la = time_mode(sp, mcb, torch, T, V, dCs, dHCs, m, max(3, args.steps // 4), 3, barrier)
+                st = max(3, args.steps // 4)
+                var[name] = {"ms_per_step": ms / st, "configs_per_s": nc / (ms / st * 1e-3)}
+                if m == mcb.MAPS:
+                    mb = 4 * nc * (c.M * c.M - c.M) + 4 * nc * tc["P"] ** 2 + unique_bytes + 2.0 * c.M * nc
+                    var[name]["map_stream_GBps"] = mb / (ms / st * 1e-3) / 1e9
+                    var[name]["hbm_frac"] = var[name]["map_stream_GBps"] / peaks["hbm_gbs"]
+                    sp.drop_structure(mcb.MAP1); sp.drop_structure(mcb.MAP2)
+            except Exception as ex:  # report, never hide
+                var[name] = {"error": str(ex)}
+        line["variants"] = var
+
+    # ---- the oracle beside it (rank 0, N=1 only) ----
+    if rank == 0 and world == 1 and not args.no_cpu:
+        import oracle
+        oracle.build()
+        v, used, nrows, dt = oracle_sample_rate(c, T, V, Cs[0], args.cpu_seconds)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": used, "kind": "oracle",
+                                "sample": f"{nrows} seeded rows of {nc} (rows are independent), {dt:.1f} s, all host threads"}
+        v1, used1, nrows1, dt1 = oracle_sample_rate(c, T, V, Cs[0], max(2.0, args.cpu_seconds / 4), nthreads=1)
+        line["cpu_baseline_1thread"] = {"value": v1, "unit": UNIT, "cores": used1, "kind": "oracle",
+                                        "sample": f"{nrows1} seeded rows, {dt1:.1f} s"}
+    sp.close()
+    if rank == 0:
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--cfg", type=int, default=2, choices=range(5))
+    ap.add_argument("--mode", default="auto", choices=sorted(MODES))
+    ap.add_argument("--impl", default="mcb", choices=["mcb", "reference"])
+    ap.add_argument("--variants", action="store_true", help="also time the other hc_apply modes (short)")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_gpu(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

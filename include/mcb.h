@@ -136,6 +136,16 @@ int  mcb_hc_apply_host(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
 /* Number of kernels the last mcb_hc_apply on this space launched (for launch accounting). */
 int  mcb_last_apply_launches(const mcb_space* sp);
 
+/* ---- measurement support: device time of each kernel of hc_apply --------------------------------------------
+ * mcb_timing_enable(sp, 1) clears the record and makes every following mcb_hc_apply on this space record CUDA
+ * events on its stream around each of its kernels (at most 512 applies are kept; later ones are not recorded);
+ * mcb_timing_enable(sp, 0) stops recording.  mcb_timing_read waits for the recorded events and writes, for the
+ * first min(recorded, max_applies) applies, ms_out[apply][3] (host float, milliseconds of kernel 0, 1, 2 in
+ * launch order; 0 for kernels the mode does not launch) and launches_out[apply] (host int).  Returns the
+ * number of applies written (>= 0) or an MCB_E* code. */
+int  mcb_timing_enable(mcb_space* sp, int on);
+int  mcb_timing_read(mcb_space* sp, int max_applies, float* ms_out, int* launches_out);
+
 /* ---- errors ------------------------------------------------------------------------------------------- */
 const char* mcb_strerror(int status);
 int         mcb_last_cuda_error(void);       /* cudaError_t of the last failing CUDA call in this thread */

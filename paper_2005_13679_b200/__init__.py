@@ -26,7 +26,7 @@ EXPORTS = (
     "mcb_space_create", "mcb_space_destroy", "mcb_nc", "mcb_nc_removed", "mcb_binom_table",
     "mcb_unrank", "mcb_rank", "mcb_structure_bytes", "mcb_build_structure", "mcb_detach_structure",
     "mcb_fock_export", "mcb_map1_export", "mcb_map2_export", "mcb_apply_workspace_bytes",
-    "mcb_hc_apply", "mcb_hc_apply_host", "mcb_last_apply_launches", "mcb_strerror", "mcb_last_cuda_error",
+    "mcb_hc_apply", "mcb_hc_apply_host", "mcb_last_apply_launches", "mcb_timing_enable", "mcb_timing_read", "mcb_strerror", "mcb_last_cuda_error",
 )
 
 _lib = None
@@ -68,6 +68,8 @@ def lib():
         L.mcb_hc_apply.argtypes = [vp, vp, vp, vp, vp, i, vp, vp]
         L.mcb_hc_apply_host.argtypes = [vp, vp, vp, vp, vp, i, vp, vp, vp, vp]
         L.mcb_last_apply_launches.argtypes = [vp]
+        L.mcb_timing_enable.argtypes = [vp, i]
+        L.mcb_timing_read.argtypes = [vp, i, vp, vp]
         L.mcb_strerror.argtypes = [i]; L.mcb_strerror.restype = ctypes.c_char_p
         L.mcb_last_cuda_error.argtypes = []
         _lib = L
@@ -243,6 +245,18 @@ class Space:
                                        mode, self._workspace["dC"].data_ptr(), self._workspace["dHC"].data_ptr(),
                                        self._ws(mode), _stream_ptr(stream)), "mcb_hc_apply_host")
         return out_host
+
+    def timing_enable(self, on: bool = True):
+        _check(lib().mcb_timing_enable(self._h, 1 if on else 0), "mcb_timing_enable")
+
+    def timing_read(self, max_applies: int = 512):
+        """(ms [applies, 3] float32, launches [applies] int32) of the applies recorded since timing_enable."""
+        ms = np.zeros((max_applies, 3), dtype=np.float32)
+        la = np.zeros(max_applies, dtype=np.int32)
+        n = lib().mcb_timing_read(self._h, max_applies, ms.ctypes.data, la.ctypes.data)
+        if n < 0:
+            raise McbError(n, "mcb_timing_read")
+        return ms[:n], la[:n]
 
     def last_apply_launches(self) -> int:
         return int(lib().mcb_last_apply_launches(self._h))

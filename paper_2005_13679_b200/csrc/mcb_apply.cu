@@ -13,6 +13,19 @@
 #include <string.h>
 #include "mcb_device.cuh"
 
+// measurement support (mcb_timing_enable): event i of the current apply's slot, recorded on the apply's stream
+static inline int mcb_tick(mcb_space* sp, int i, cudaStream_t st)
+{
+    if (!sp->timing || sp->t_count >= MCB_TIMING_RING) return MCB_OK;
+    MCB_CUDA(cudaEventRecord(sp->t_ev[sp->t_count][i], st));
+    return MCB_OK;
+}
+static inline void mcb_tick_done(mcb_space* sp, int launches)
+{
+    if (!sp->timing || sp->t_count >= MCB_TIMING_RING) return;
+    sp->t_launches[sp->t_count++] = launches;
+}
+
 // =========================================================================================================
 // host: packing of T, V
 // =========================================================================================================
@@ -505,6 +518,7 @@ static int launch_direct(mcb_space* sp, bool use_maps, const mcb_c128* T, const 
     a.map1 = sp->d_map1; a.ld1 = sp->map1_ld; a.map2 = sp->d_map2; a.ld2 = sp->map2_ld;
     const int threads = 128;
     const unsigned blocks = (unsigned)((sp->nc + threads - 1) / threads);
+    { int rc = mcb_tick(sp, 0, st); if (rc) return rc; }
     if (use_maps) {
         MCB_CUDA(cudaFuncSetAttribute(k_hc_direct<M, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
         k_hc_direct<M, true><<<blocks, threads, bytes, st>>>(a);
@@ -513,6 +527,8 @@ static int launch_direct(mcb_space* sp, bool use_maps, const mcb_c128* T, const 
         k_hc_direct<M, false><<<blocks, threads, bytes, st>>>(a);
     }
     MCB_CHECK_LAUNCH();
+    { int rc = mcb_tick(sp, 1, st); if (rc) return rc; }
+    mcb_tick_done(sp, 1);
     sp->last_launches = 1;
     return MCB_OK;
 }
@@ -561,11 +577,15 @@ static int launch_gemm(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
     }
     int grid = sm_count * ctas_per_sm;
     if (grid > g.ntiles) grid = g.ntiles;
+    { int rc = mcb_tick(sp, 0, st); if (rc) return rc; }
     k_hc2_contract<M><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(g);
     MCB_CHECK_LAUNCH();
+    { int rc = mcb_tick(sp, 1, st); if (rc) return rc; }
     const int threads = 256;
     k_hc2_reduce<M><<<(unsigned)((sp->nc + threads - 1) / threads), threads, 0, st>>>(g);
     MCB_CHECK_LAUNCH();
+    { int rc = mcb_tick(sp, 2, st); if (rc) return rc; }
+    mcb_tick_done(sp, 2);
     sp->last_launches = 2;
     return MCB_OK;
 }

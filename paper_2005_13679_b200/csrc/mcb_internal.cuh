@@ -4,6 +4,9 @@
 #include <stdint.h>
 #include "mcb.h"
 
+#define MCB_TIMING_RING 512
+#define MCB_MAX_APPLY_KERNELS 3
+
 // ---- device-side view of the small per-space constants -------------------------------------------------
 // G[j][s] = binom(s + j, j + 1), j = 0..M-2, s = 0..N: the number of configurations that precede, in the
 // order of Eq. (14), every configuration whose prefix sum S_j = n_0 + .. + n_j equals s
@@ -41,6 +44,11 @@ struct mcb_space {
     void* d_coef; size_t coef_bytes;
     void* h_coef;              // host scratch for packing
     int last_launches;
+    // optional per-kernel timing (mcb_timing_enable): ring of event tuples, one per apply
+    int timing;                          // 0 = off
+    int t_count;                         // applies recorded since enable (saturates at MCB_TIMING_RING)
+    cudaEvent_t t_ev[MCB_TIMING_RING][MCB_MAX_APPLY_KERNELS + 1];
+    int t_launches[MCB_TIMING_RING];
 };
 
 static inline long long mcb_round_up(long long x, long long a) { return (x + a - 1) / a * a; }

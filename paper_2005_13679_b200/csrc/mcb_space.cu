@@ -116,6 +116,9 @@ extern "C" int mcb_space_create(int N, int M, mcb_space** out)
 extern "C" void mcb_space_destroy(mcb_space* sp)
 {
     if (!sp) return;
+    for (int i = 0; i < MCB_TIMING_RING; ++i)
+        for (int j = 0; j <= MCB_MAX_APPLY_KERNELS; ++j)
+            if (sp->t_ev[i][j]) cudaEventDestroy(sp->t_ev[i][j]);
     if (sp->d_consts) cudaFree(sp->d_consts);
     if (sp->d_coef) cudaFree(sp->d_coef);
     free(sp->h_coef);
@@ -273,3 +276,34 @@ extern "C" int mcb_map2_export(const mcb_space* sp, long long b0, long long coun
 }
 
 extern "C" int mcb_last_apply_launches(const mcb_space* sp) { return sp ? sp->last_launches : -1; }
+
+// ---- per-kernel timing of hc_apply (measurement support) ----------------------------------------------------
+extern "C" int mcb_timing_enable(mcb_space* sp, int on)
+{
+    if (!sp) return MCB_EINVAL;
+    if (on) {
+        for (int i = 0; i < MCB_TIMING_RING; ++i)
+            for (int j = 0; j <= MCB_MAX_APPLY_KERNELS; ++j)
+                if (!sp->t_ev[i][j]) MCB_CUDA(cudaEventCreate(&sp->t_ev[i][j]));
+        sp->t_count = 0;
+    }
+    sp->timing = on ? 1 : 0;
+    return MCB_OK;
+}
+
+extern "C" int mcb_timing_read(mcb_space* sp, int max_applies, float* ms_out, int* launches_out)
+{
+    if (!sp || max_applies < 0 || (max_applies > 0 && (!ms_out || !launches_out))) return MCB_EINVAL;
+    int n = sp->t_count < max_applies ? sp->t_count : max_applies;
+    for (int i = 0; i < n; ++i) {
+        const int L = sp->t_launches[i];
+        MCB_CUDA(cudaEventSynchronize(sp->t_ev[i][L]));
+        for (int j = 0; j < MCB_MAX_APPLY_KERNELS; ++j) {
+            float ms = 0.0f;
+            if (j < L) MCB_CUDA(cudaEventElapsedTime(&ms, sp->t_ev[i][j], sp->t_ev[i][j + 1]));
+            ms_out[(size_t)i * MCB_MAX_APPLY_KERNELS + j] = ms;
+        }
+        launches_out[i] = L;
+    }
+    return n;
+}
