@@ -67,7 +67,7 @@ def term_counts(N: int, M: int, nc: int, nc1: int, nc2: int):
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md clocks line)."""
 
-    def __init__(self, index: int, period_s: float = 0.05):
+    def __init__(self, index: int, period_s: float = 0.005):
         self.index, self.period = index, period_s
         self.samples, self.reasons = [], set()
         self.max_mhz = None
@@ -197,6 +197,41 @@ def config_dict(c, variant: str):
 
 
 # ------------------------------------------------------------------------------------------------------------
+# multi-process plumbing: N independent replicas (the path does not shard); the only
+# cross-rank operations are the barrier around the timed region and the max of the per-rank device times.
+# ------------------------------------------------------------------------------------------------------------
+class Job:
+    def __init__(self, world: int, backend: str, device):
+        self.world, self.device, self.dist = world, device, None
+        if world > 1:
+            import torch.distributed as dist
+            kw = {"device_id": device} if backend == "nccl" else {}
+            dist.init_process_group(backend, **kw)
+            self.dist = dist
+
+    def barrier(self):
+        if self.dist is not None:
+            self.dist.barrier()
+
+    def max_over_ranks(self, x: float) -> float:
+        if self.dist is None:
+            return x
+        import torch
+        t = torch.tensor([x], dtype=torch.float64, device=self.device)
+        self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def whole_job_value(self, units_per_rank: float, ms_per_step_this_rank: float) -> float:
+        """units all ranks processed / max-over-ranks time (weak scaling, replicas)."""
+        ms = self.max_over_ranks(ms_per_step_this_rank)
+        return self.world * units_per_rank / (ms * 1e-3)
+
+    def close(self):
+        if self.dist is not None:
+            self.dist.destroy_process_group()
+
+
+# ------------------------------------------------------------------------------------------------------------
 # GPU arm
 # ------------------------------------------------------------------------------------------------------------
 MODES = {"auto": 0, "maps": 1, "rehash": 2, "gemm": 3}
@@ -236,21 +271,8 @@ def run_gpu(args):
         raise RuntimeError("bench.py needs a CUDA device: libmcb has no CPU path")
     mcb.lib()
     torch.cuda.set_device(local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-
-    def barrier():
-        if dist is not None:
-            dist.barrier()
-
-    def max_over_ranks(x: float) -> float:
-        if dist is None:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+    job = Job(world, "nccl", torch.device("cuda", local))
+    barrier, max_over_ranks = job.barrier, job.max_over_ranks
 
     peaks = load_peaks()
     R = 3
@@ -286,9 +308,8 @@ def run_gpu(args):
     clocks.start()
     ms_total, kms, launches = time_mode(sp, mcb, torch, T, V, dCs, dHCs, mode, args.steps, args.warmup, barrier)
     clk = clocks.stop()
-    ms_total = max_over_ranks(ms_total)
-    ms_step = ms_total / args.steps
-    value = world * nc / (ms_step * 1e-3)
+    ms_step = max_over_ranks(ms_total) / args.steps
+    value = job.whole_job_value(nc, ms_total / args.steps)
 
     # ---- end to end through the public API with HOST buffers (pinned), H2D + D2H inside the timed region ----
     hC = [torch.from_numpy(C).pin_memory() for C in Cs]
@@ -389,8 +410,7 @@ def run_gpu(args):
     sp.close()
     if rank == 0:
         print(json.dumps(line))
-    if dist is not None:
-        dist.destroy_process_group()
+    job.close()
     return 0
 
 

@@ -146,6 +146,11 @@ int  mcb_last_apply_launches(const mcb_space* sp);
 int  mcb_timing_enable(mcb_space* sp, int on);
 int  mcb_timing_read(mcb_space* sp, int max_applies, float* ms_out, int* launches_out);
 
+/* FP64 throughput the current device sustains, measured with register-only kernels on `stream` (synchronous):
+ * kind 0 = DFMA chains (plain FP64 pipe), 1 = DMMA m8n8k4 chains (FP64 tensor path), 2 = both interleaved.
+ * *tflops_out (host) receives TFLOP/s.  Allocates and frees 8 bytes of device memory internally. */
+int  mcb_fp64_peak(int kind, double* tflops_out, void* stream);
+
 /* ---- errors ------------------------------------------------------------------------------------------- */
 const char* mcb_strerror(int status);
 int         mcb_last_cuda_error(void);       /* cudaError_t of the last failing CUDA call in this thread */

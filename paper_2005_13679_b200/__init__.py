@@ -26,7 +26,7 @@ EXPORTS = (
     "mcb_space_create", "mcb_space_destroy", "mcb_nc", "mcb_nc_removed", "mcb_binom_table",
     "mcb_unrank", "mcb_rank", "mcb_structure_bytes", "mcb_build_structure", "mcb_detach_structure",
     "mcb_fock_export", "mcb_map1_export", "mcb_map2_export", "mcb_apply_workspace_bytes",
-    "mcb_hc_apply", "mcb_hc_apply_host", "mcb_last_apply_launches", "mcb_timing_enable", "mcb_timing_read", "mcb_strerror", "mcb_last_cuda_error",
+    "mcb_hc_apply", "mcb_hc_apply_host", "mcb_last_apply_launches", "mcb_timing_enable", "mcb_timing_read", "mcb_fp64_peak", "mcb_strerror", "mcb_last_cuda_error",
 )
 
 _lib = None
@@ -70,6 +70,7 @@ def lib():
         L.mcb_last_apply_launches.argtypes = [vp]
         L.mcb_timing_enable.argtypes = [vp, i]
         L.mcb_timing_read.argtypes = [vp, i, vp, vp]
+        L.mcb_fp64_peak.argtypes = [i, ctypes.POINTER(ctypes.c_double), vp]
         L.mcb_strerror.argtypes = [i]; L.mcb_strerror.restype = ctypes.c_char_p
         L.mcb_last_cuda_error.argtypes = []
         _lib = L
@@ -99,6 +100,13 @@ def _host_c128(a, shape) -> np.ndarray:
     if a.size != int(np.prod(shape)):
         raise ValueError(f"expected {shape} complex values, got {a.shape}")
     return a
+
+
+def fp64_peak(kind: int = 0, stream=None) -> float:
+    """Measured FP64 TFLOP/s of the current device: kind 0 DFMA, 1 DMMA m8n8k4, 2 both interleaved."""
+    out = ctypes.c_double(0.0)
+    _check(lib().mcb_fp64_peak(kind, ctypes.byref(out), _stream_ptr(stream)), "mcb_fp64_peak")
+    return float(out.value)
 
 
 class Space:
