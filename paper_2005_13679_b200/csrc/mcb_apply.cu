@@ -10,21 +10,9 @@
 //                          F(m,ql) = sqrt((m_q+1)(m_l+1+[q==l])), so that per intermediate m the work is a dense
 //                          P x P complex mat-vec -- batched over m: an FP64 tensor-core (DMMA) GEMM with the
 //                          packed V stationary in registers.  T rides along inside V (sum_s a+_s a_s = N).
+#include <stdlib.h>
 #include <string.h>
 #include "mcb_device.cuh"
-
-// measurement support (mcb_timing_enable): event i of the current apply's slot, recorded on the apply's stream
-static inline int mcb_tick(mcb_space* sp, int i, cudaStream_t st)
-{
-    if (!sp->timing || sp->t_count >= MCB_TIMING_RING) return MCB_OK;
-    MCB_CUDA(cudaEventRecord(sp->t_ev[sp->t_count][i], st));
-    return MCB_OK;
-}
-static inline void mcb_tick_done(mcb_space* sp, int launches)
-{
-    if (!sp->timing || sp->t_count >= MCB_TIMING_RING) return;
-    sp->t_launches[sp->t_count++] = launches;
-}
 
 // =========================================================================================================
 // host: packing of T, V
@@ -35,7 +23,7 @@ static inline void mcb_tick_done(mcb_space* sp, int launches)
 // so the ordered sum of Eq. (13) equals the sum over unordered pairs of Vp times the operator (reading A8).
 // With fold_T, Veff = V + (2/(N-1)) T[k][l] delta_sq, which adds sum_kl T_kl a+_k (N^ ) a_l / (N-1) = the one-body
 // term on N-particle states.
-static void pack_pairs(int N, int M, const mcb_c128* T, const mcb_c128* V, bool fold_T, double* vr, double* vi /* [P][P] */)
+void mcb_pack_pairs(int N, int M, const mcb_c128* T, const mcb_c128* V, bool fold_T, double* vr, double* vi /* [P][P] */)
 {
     const int P = M * (M + 1) / 2;
     const double tf = (fold_T && N >= 2) ? 2.0 / (double)(N - 1) : 0.0;
@@ -202,268 +190,6 @@ __global__ void __launch_bounds__(128) k_hc_direct(DirectArgs p)
 }
 
 // =========================================================================================================
-// MCB_GEMM path
-// =========================================================================================================
-// Tile shape per M (compile time).  The packed coefficient matrix A is STATIONARY IN REGISTERS as DMMA
-// m8n8k4 A-fragments: warp (wr, wc) of a CTA owns row blocks {wr, wr + WR, ..} (8 rows each) for ALL k-steps and
-// sweeps the column blocks (8 intermediates m each) {wc, wc + WC, ..} of the CTA's tile of TM intermediates.
-//   EMBED (small M): the complex P x P product is embedded as a real 2P x 2P one,
-//        [Wr; Wi] = [[Vr, -Vi], [Vi, Vr]] . [Dr; Di], which pads 2P (not P) to the 8 x 4 fragment grid;
-//   otherwise: real fragments of Vr, Vi and three accumulators (Vr.Dr, Vi.Di, Vr.Di + Vi.Dr).
-constexpr int cmax(int a, int b) { return a > b ? a : b; }
-constexpr int cdiv(int a, int b) { return (a + b - 1) / b; }
-
-template <int M> struct GemmCfg {
-    static constexpr int P = M * (M + 1) / 2;
-    static constexpr bool EMBED = (M <= 8);
-    static constexpr int ROWS = EMBED ? 2 * P : P;          // output rows of the real GEMM(s)
-    static constexpr int RB = cdiv(ROWS, 8);                // 8-row blocks
-    static constexpr int KD = EMBED ? 2 * P : P;            // contraction length
-    static constexpr int NK = cdiv(KD, 4);                  // k-steps of 4
-    static constexpr int PER = EMBED ? 1 : 2;               // A doubles per (row block, k-step, lane)
-    static constexpr int NRB_MAX = cmax(1, 48 / (NK * PER));
-    static constexpr int WR = cdiv(RB, NRB_MAX);
-    static constexpr int NRB = cdiv(RB, WR);
-    static constexpr int WC = WR >= 4 ? 1 : (WR >= 2 ? 2 : 4);
-    static constexpr int TM = 128;                          // intermediates per tile
-    static constexpr int LD = TM + 4;                       // smem row stride (doubles): LD % 16 == 4 -> conflict-free B frags
-    static constexpr int THREADS = WR * WC * 32;
-    static constexpr int NPARTS = cmax(1, THREADS / TM);    // gather: threads per intermediate
-    static constexpr int DROWS = NK * 4;                    // rows of each staged D plane
-    static constexpr int NPLANES = EMBED ? 1 : 2;
-    static constexpr int A_ROWS = RB * 8, A_COLS = NK * 4;  // padded coefficient matrix (row-major), x PER matrices
-    static constexpr size_t SMEM = (size_t)(NPLANES * DROWS * LD + 2 * M * TM) * sizeof(double);
-    static_assert(THREADS >= TM || TM % THREADS == 0, "gather mapping");
-};
-
-struct GemmArgs {
-    McbDev d;
-    McbFockView fock;
-    const double2* C;
-    double2* HC;
-    const double* A;           // EMBED: [A_ROWS][A_COLS]; else Vr [A_ROWS][A_COLS] then Vi [A_ROWS][A_COLS]
-    double* W;                 // [P][2][ldw]: W'[ks][re|im][m] = F(m,ks) * sum_ql Vp[ks][ql] F(m,ql) C[m + e_q + e_l]
-    long long ldw;
-    int ntiles;
-};
-
-__device__ __forceinline__ void dmma884(double& c0, double& c1, const double a, const double b)
-{
-    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
-                 : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
-}
-
-// pair index -> (k, s), k <= s, order (0,0),(0,1),..
-__device__ __forceinline__ void pair_decode(int M, int a, int& k, int& s)
-{
-    k = 0;
-    int len = M;
-    while (a >= len) { a -= len; --len; ++k; }
-    s = k + a;
-}
-
-template <int M>
-__global__ void __launch_bounds__(GemmCfg<M>::THREADS, 1) k_hc2_contract(GemmArgs p)
-{
-    using Cfg = GemmCfg<M>;
-    constexpr int P = Cfg::P, NK = Cfg::NK, NRB = Cfg::NRB, WR = Cfg::WR, WC = Cfg::WC, TM = Cfg::TM, LD = Cfg::LD;
-    constexpr bool EMBED = Cfg::EMBED;
-    extern __shared__ double smem[];
-    double* Dr = smem;                                       // [DROWS][LD]   (EMBED: rows 0..P-1 real, P..2P-1 imag)
-    double* Di = smem + Cfg::DROWS * LD;                     // [DROWS][LD]   (non-EMBED only)
-    double* R1 = smem + Cfg::NPLANES * Cfg::DROWS * LD;      // [M][TM]  sqrt(m_j + 1)
-    double* R2 = R1 + M * TM;                                // [M][TM]  sqrt((m_j + 1)(m_j + 2))
-    const McbDev& d = p.d;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int wr = warp % WR, wc = warp / WR;
-    const int grp = lane >> 2, tig = lane & 3;
-
-    // ---- stationary A fragments: a[rb][ks] = A[(rbg*8 + grp)][ks*4 + tig] ----
-    double a_re[NRB][NK];
-    double a_im[EMBED ? 1 : NRB][EMBED ? 1 : NK];
-    int row_k[NRB], row_s[NRB], row_part[NRB];               // which W' row this lane's accumulator rows are
-#pragma unroll
-    for (int i = 0; i < NRB; ++i) {
-        const int rbg = wr + i * WR;
-        const int r = rbg * 8 + grp;
-        const bool live = rbg < Cfg::RB;
-#pragma unroll
-        for (int ks = 0; ks < NK; ++ks) {
-            a_re[i][ks] = live ? p.A[(size_t)r * Cfg::A_COLS + ks * 4 + tig] : 0.0;
-            if (!EMBED) a_im[i][ks] = live ? p.A[(size_t)(Cfg::A_ROWS + r) * Cfg::A_COLS + ks * 4 + tig] : 0.0;
-        }
-        int pr = -1, part = 0;
-        if (live && r < Cfg::ROWS) { pr = EMBED ? (r % P) : r; part = EMBED ? (r / P) : 0; }
-        int k = 0, s = 0;
-        if (pr >= 0) pair_decode(M, pr, k, s);
-        row_k[i] = pr >= 0 ? k : -1; row_s[i] = s; row_part[i] = part;
-    }
-    // zero the padding rows of the staged planes once (never written again)
-    for (int i = tid; i < Cfg::NPLANES * Cfg::DROWS * LD; i += Cfg::THREADS) smem[i] = 0.0;
-    __syncthreads();
-
-    const int m_local = tid % TM;
-    const int part = tid / TM;
-
-    for (int tile = blockIdx.x; tile < p.ntiles; tile += gridDim.x) {
-        const int m0 = tile * TM;
-        // ================= gather: D[ql][m] = F(m,ql) C[index(m + e_q + e_l)] =================
-        if (part < Cfg::NPARTS) {
-            const int m = m0 + m_local;
-            const bool valid = m < d.nc2;
-            int X[M], Y[M];
-            double r1[M], r2[M];
-            {
-                int A1[M], A2[M];
-                int run = 0, x = 0, tot1 = 0;
-#pragma unroll
-                for (int j = 0; j < M; ++j) {
-                    const int nj = valid ? (int)p.fock.occ2[(long long)j * p.fock.ld2 + m] : 0;
-                    run += nj;
-                    r1[j] = __ldg(d.sq + nj + 1);
-                    r2[j] = __ldg(d.sq2 + nj + 2);
-                    X[j] = x;
-                    if (j <= M - 2) {
-                        const int a0 = mcb_ldG(d.G, d.ldg, j, run);
-                        A1[j] = mcb_ldG(d.G, d.ldg, j, run + 1);
-                        A2[j] = mcb_ldG(d.G, d.ldg, j, run + 2);
-                        x += a0 - A1[j]; tot1 += A1[j];
-                    } else { A1[j] = 0; A2[j] = 0; }
-                }
-                int pre = tot1, suf = 0;
-#pragma unroll
-                for (int l = M - 1; l >= 0; --l) { pre -= A1[l]; suf += A2[l]; Y[l] = pre + suf; }
-            }
-            if (part == 0) {
-#pragma unroll
-                for (int j = 0; j < M; ++j) { R1[j * TM + m_local] = r1[j]; R2[j * TM + m_local] = r2[j]; }
-            }
-            int c = 0;
-#pragma unroll
-            for (int q = 0; q < M; ++q) {
-#pragma unroll
-                for (int l = q; l < M; ++l, ++c) {
-                    if (Cfg::NPARTS == 1 || (c % Cfg::NPARTS) == part) {
-                        const int tgt = d.nc - 1 - X[q] - Y[l];
-                        double2 z = make_double2(0.0, 0.0);
-                        if (valid) z = __ldg(p.C + tgt);
-                        const double f = (q == l) ? r2[q] : r1[q] * r1[l];
-                        if (EMBED) { Dr[c * LD + m_local] = f * z.x; Dr[(P + c) * LD + m_local] = f * z.y; }
-                        else       { Dr[c * LD + m_local] = f * z.x; Di[c * LD + m_local] = f * z.y; }
-                    }
-                }
-            }
-        }
-        __syncthreads();
-
-        // ================= contraction on the FP64 tensor cores + scaled store =================
-        for (int cb = wc * 2; cb < TM / 8; cb += WC * 2) {
-            double acc[NRB][2][EMBED ? 1 : 3][2];
-#pragma unroll
-            for (int i = 0; i < NRB; ++i)
-#pragma unroll
-                for (int j = 0; j < 2; ++j)
-#pragma unroll
-                    for (int t = 0; t < (EMBED ? 1 : 3); ++t) { acc[i][j][t][0] = 0.0; acc[i][j][t][1] = 0.0; }
-            const double* b_base = Dr + tig * LD + cb * 8 + grp;
-#pragma unroll
-            for (int ks = 0; ks < NK; ++ks) {
-                const double br0 = b_base[ks * 4 * LD], br1 = b_base[ks * 4 * LD + 8];
-                double bi0 = 0.0, bi1 = 0.0;
-                if (!EMBED) { bi0 = b_base[Cfg::DROWS * LD + ks * 4 * LD]; bi1 = b_base[Cfg::DROWS * LD + ks * 4 * LD + 8]; }
-#pragma unroll
-                for (int i = 0; i < NRB; ++i) {
-                    if (EMBED) {
-                        dmma884(acc[i][0][0][0], acc[i][0][0][1], a_re[i][ks], br0);
-                        dmma884(acc[i][1][0][0], acc[i][1][0][1], a_re[i][ks], br1);
-                    } else {
-                        dmma884(acc[i][0][0][0], acc[i][0][0][1], a_re[i][ks], br0);
-                        dmma884(acc[i][1][0][0], acc[i][1][0][1], a_re[i][ks], br1);
-                        dmma884(acc[i][0][1][0], acc[i][0][1][1], a_im[i][ks], bi0);
-                        dmma884(acc[i][1][1][0], acc[i][1][1][1], a_im[i][ks], bi1);
-                        dmma884(acc[i][0][2][0], acc[i][0][2][1], a_re[i][ks], bi0);
-                        dmma884(acc[i][1][2][0], acc[i][1][2][1], a_re[i][ks], bi1);
-                        dmma884(acc[i][0][2][0], acc[i][0][2][1], a_im[i][ks], br0);
-                        dmma884(acc[i][1][2][0], acc[i][1][2][1], a_im[i][ks], br1);
-                    }
-                }
-            }
-            // epilogue: W'[ks][part][m] = F(m,ks) * acc;  this lane holds columns col, col+1 of row (rbg*8 + grp)
-#pragma unroll
-            for (int i = 0; i < NRB; ++i) {
-                if (row_k[i] < 0) continue;
-                const int k = row_k[i], s = row_s[i];
-                const int pr = mcb_pair_index(M, k, s);
-#pragma unroll
-                for (int j = 0; j < 2; ++j) {
-                    const int col = (cb + j) * 8 + tig * 2;
-                    double f0, f1;
-                    if (k == s) { f0 = R2[k * TM + col]; f1 = R2[k * TM + col + 1]; }
-                    else { f0 = R1[k * TM + col] * R1[s * TM + col]; f1 = R1[k * TM + col + 1] * R1[s * TM + col + 1]; }
-                    if (EMBED) {
-                        double2 o = make_double2(f0 * acc[i][j][0][0], f1 * acc[i][j][0][1]);
-                        *reinterpret_cast<double2*>(p.W + ((size_t)pr * 2 + row_part[i]) * p.ldw + m0 + col) = o;
-                    } else {
-                        double2 ore = make_double2(f0 * (acc[i][j][0][0] - acc[i][j][1][0]), f1 * (acc[i][j][0][1] - acc[i][j][1][1]));
-                        double2 oim = make_double2(f0 * acc[i][j][2][0], f1 * acc[i][j][2][1]);
-                        *reinterpret_cast<double2*>(p.W + ((size_t)pr * 2 + 0) * p.ldw + m0 + col) = ore;
-                        *reinterpret_cast<double2*>(p.W + ((size_t)pr * 2 + 1) * p.ldw + m0 + col) = oim;
-                    }
-                }
-            }
-        }
-        __syncthreads();               // the next tile's gather overwrites D, R1, R2
-    }
-}
-
-// HC[g] = sum over allowed removal pairs (k<=s) of W'[ks][index2(n^g - e_k - e_s)]: every W' element is read by
-// exactly one g, so there are no atomics on the output.  One thread per output configuration.
-template <int M>
-__global__ void __launch_bounds__(256) k_hc2_reduce(GemmArgs p)
-{
-    const McbDev& d = p.d;
-    const int g = blockIdx.x * blockDim.x + threadIdx.x;
-    if (g >= d.nc) return;
-    int n[M], X[M], Y[M];
-    {
-        int A1[M], A2[M];
-        int run = 0, x = 0, tot1 = 0;
-#pragma unroll
-        for (int j = 0; j < M; ++j) {
-            n[j] = p.fock.occ[(long long)j * p.fock.ld + g];
-            run += n[j];
-            X[j] = x;
-            if (j <= M - 2) {
-                // prefix sums of n - e_k - e_s: S_j (j < k), S_j - 1 (k <= j < s), S_j - 2 (j >= s)
-                const int a0 = mcb_ldG(d.G, d.ldg, j, run);
-                A1[j] = mcb_ldG(d.G, d.ldg, j, run >= 1 ? run - 1 : 0);
-                A2[j] = mcb_ldG(d.G, d.ldg, j, run >= 2 ? run - 2 : 0);
-                x += a0 - A1[j]; tot1 += A1[j];
-            } else { A1[j] = 0; A2[j] = 0; }
-        }
-        int pre = tot1, suf = 0;
-#pragma unroll
-        for (int l = M - 1; l >= 0; --l) { pre -= A1[l]; suf += A2[l]; Y[l] = pre + suf; }
-    }
-    double re = 0.0, im = 0.0;
-    int a = 0;
-#pragma unroll
-    for (int k = 0; k < M; ++k) {
-#pragma unroll
-        for (int s = k; s < M; ++s, ++a) {
-            const bool ok = (k == s) ? (n[k] >= 2) : (n[k] >= 1 && n[s] >= 1);
-            if (ok) {
-                const int mi = d.nc2 - 1 - X[k] - Y[s];
-                const double* w = p.W + (size_t)a * 2 * p.ldw + mi;
-                re += __ldg(w);
-                im += __ldg(w + p.ldw);
-            }
-        }
-    }
-    p.HC[g] = make_double2(re, im);
-}
-
-// =========================================================================================================
 // host entry points
 // =========================================================================================================
 #define MCB_DISPATCH_APPLY_M(M, CALL)                                                                    \
@@ -484,8 +210,6 @@ static int resolve_mode(const mcb_space* sp, int mode)
     return mode;
 }
 
-static long long gemm_ldw(const mcb_space* sp) { return mcb_round_up(sp->nc2, 128); }
-
 extern "C" long long mcb_apply_workspace_bytes(const mcb_space* sp, int mode)
 {
     if (!sp) return MCB_EINVAL;
@@ -493,7 +217,7 @@ extern "C" long long mcb_apply_workspace_bytes(const mcb_space* sp, int mode)
     if (mode < MCB_AUTO || mode > MCB_GEMM) return MCB_EINVAL;
     mode = resolve_mode(sp, mode);
     if (mode != MCB_GEMM) return 0;
-    return (long long)sp->P * 2 * gemm_ldw(sp) * (long long)sizeof(double);
+    return mcb_gemm_workspace_bytes(sp);
 }
 
 template <int M>
@@ -507,7 +231,7 @@ static int launch_direct(mcb_space* sp, bool use_maps, const mcb_c128* T, const 
     {
         double* vr = h + 2 * (M * M + P * P);               // scratch behind the packed block
         double* vi = vr + P * P;
-        pack_pairs(sp->N, M, T, V, false, vr, vi);
+        mcb_pack_pairs(sp->N, M, T, V, false, vr, vi);
         for (int i = 0; i < P * P; ++i) { h[2 * (M * M + i)] = vr[i]; h[2 * (M * M + i) + 1] = vi[i]; }
     }
     const size_t bytes = sizeof(mcb_c128) * (size_t)(M * M + P * P);
@@ -533,63 +257,6 @@ static int launch_direct(mcb_space* sp, bool use_maps, const mcb_c128* T, const 
     return MCB_OK;
 }
 
-template <int M>
-static int launch_gemm(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
-                       const mcb_c128* d_C, mcb_c128* d_HC, void* d_ws, cudaStream_t st)
-{
-    using Cfg = GemmCfg<M>;
-    constexpr int P = Cfg::P;
-    // ---- coefficient matrix in the padded fragment grid ----
-    double* h = (double*)sp->h_coef;
-    const size_t mat = (size_t)Cfg::A_ROWS * Cfg::A_COLS;
-    const size_t a_bytes = sizeof(double) * mat * Cfg::PER;
-    double* vr = h + mat * Cfg::PER;
-    double* vi = vr + P * P;
-    if ((char*)(vi + P * P) > (char*)sp->h_coef + sp->coef_bytes) return MCB_ENOMEM;
-    pack_pairs(sp->N, M, T, V, true, vr, vi);
-    memset(h, 0, a_bytes);
-    for (int a = 0; a < P; ++a)
-        for (int c = 0; c < P; ++c) {
-            const double re = vr[a * P + c], im = vi[a * P + c];
-            if (Cfg::EMBED) {
-                h[(size_t)a * Cfg::A_COLS + c] = re;            h[(size_t)a * Cfg::A_COLS + P + c] = -im;
-                h[(size_t)(P + a) * Cfg::A_COLS + c] = im;      h[(size_t)(P + a) * Cfg::A_COLS + P + c] = re;
-            } else {
-                h[(size_t)a * Cfg::A_COLS + c] = re;
-                h[mat + (size_t)a * Cfg::A_COLS + c] = im;
-            }
-        }
-    MCB_CUDA(cudaMemcpyAsync(sp->d_coef, h, a_bytes, cudaMemcpyHostToDevice, st));
-
-    GemmArgs g;
-    g.d = sp->dev; g.fock = sp->fock;
-    g.C = (const double2*)d_C; g.HC = (double2*)d_HC;
-    g.A = (const double*)sp->d_coef;
-    g.W = (double*)d_ws; g.ldw = gemm_ldw(sp);
-    g.ntiles = (int)((sp->nc2 + Cfg::TM - 1) / Cfg::TM);
-
-    static int sm_count = 0, ctas_per_sm = 0;
-    if (!sm_count) {
-        MCB_CUDA(cudaFuncSetAttribute(k_hc2_contract<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
-        MCB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, k_hc2_contract<M>, Cfg::THREADS, Cfg::SMEM));
-        MCB_CUDA(cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, sp->device));
-        if (ctas_per_sm < 1) return MCB_EUNSUPPORTED;
-    }
-    int grid = sm_count * ctas_per_sm;
-    if (grid > g.ntiles) grid = g.ntiles;
-    { int rc = mcb_tick(sp, 0, st); if (rc) return rc; }
-    k_hc2_contract<M><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(g);
-    MCB_CHECK_LAUNCH();
-    { int rc = mcb_tick(sp, 1, st); if (rc) return rc; }
-    const int threads = 256;
-    k_hc2_reduce<M><<<(unsigned)((sp->nc + threads - 1) / threads), threads, 0, st>>>(g);
-    MCB_CHECK_LAUNCH();
-    { int rc = mcb_tick(sp, 2, st); if (rc) return rc; }
-    mcb_tick_done(sp, 2);
-    sp->last_launches = 2;
-    return MCB_OK;
-}
-
 extern "C" int mcb_hc_apply(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
                             const mcb_c128* d_C, mcb_c128* d_HC, int mode, void* d_workspace, void* stream)
 {
@@ -608,7 +275,7 @@ extern "C" int mcb_hc_apply(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
     if (mode == MCB_MAPS && (!sp->d_map1 || (sp->N >= 2 && !sp->d_map2))) return MCB_ENOTREADY;
     if (mode == MCB_GEMM) {
         if (!d_workspace || (((uintptr_t)d_workspace) & 255)) return MCB_EINVAL;
-        MCB_DISPATCH_APPLY_M(sp->M, return launch_gemm<MT>(sp, T, V, d_C, d_HC, d_workspace, st));
+        return mcb_launch_gemm(sp, T, V, d_C, d_HC, d_workspace, st);
     } else {
         const bool use_maps = mode == MCB_MAPS;
         MCB_DISPATCH_APPLY_M(sp->M, return launch_direct<MT>(sp, use_maps, T, V, d_C, d_HC, st));

@@ -67,3 +67,24 @@ int mcb_launch_rank(const mcb_space* sp, const int* d_occ, long long batch, int*
 int mcb_launch_fock_table(const mcb_space* sp, int removed, uint16_t* d_out, long long ld, cudaStream_t st);
 int mcb_launch_map1(const mcb_space* sp, int* d_out, long long ld, cudaStream_t st);
 int mcb_launch_map2(const mcb_space* sp, int* d_out, long long ld, cudaStream_t st);
+
+// ---- hc_apply internals shared by mcb_apply.cu (direct modes) and mcb_apply_gemm.cu (GEMM mode) ----------------
+// Vp[a][c] (a = pair(k<=s), c = pair(q<=l)): the bosonic-symmetric part of V, optionally with T folded in
+void mcb_pack_pairs(int N, int M, const mcb_c128* T, const mcb_c128* V, bool fold_T, double* vr, double* vi);
+long long mcb_gemm_workspace_bytes(const mcb_space* sp);
+int mcb_launch_gemm(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, const mcb_c128* d_C, mcb_c128* d_HC,
+                    void* d_ws, cudaStream_t st);
+
+// measurement support (mcb_timing_enable): event i of the current apply's slot, recorded on the apply's stream
+static inline int mcb_tick(mcb_space* sp, int i, cudaStream_t st)
+{
+    if (!sp->timing || sp->t_count >= MCB_TIMING_RING) return MCB_OK;
+    MCB_CUDA(cudaEventRecord(sp->t_ev[sp->t_count][i], st));
+    return MCB_OK;
+}
+static inline void mcb_tick_done(mcb_space* sp, int launches)
+{
+    if (!sp->timing || sp->t_count >= MCB_TIMING_RING) return;
+    sp->t_launches[sp->t_count++] = launches;
+}
+
