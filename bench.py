@@ -234,8 +234,10 @@ class Job:
 # ------------------------------------------------------------------------------------------------------------
 # GPU arm
 # ------------------------------------------------------------------------------------------------------------
-MODES = {"auto": 0, "maps": 1, "rehash": 2, "gemm": 3}
-KERNELS = {1: ["k_hc_direct<M,maps>"], 2: ["k_hc_direct<M,rehash>"], 3: ["k_hc2_contract<M>", "k_hc2_reduce<M>"]}
+MODES = {"auto": 0, "maps": 1, "rehash": 2, "gemm": 3, "fma": 4}
+MODE_NAMES = {1: "MAPS", 2: "REHASH", 3: "GEMM", 4: "FMA"}
+KERNELS = {1: ["k_hc_direct<M,maps>"], 2: ["k_hc_direct<M,rehash>"], 3: ["k_hc2_contract<M>", "k_hc2_reduce<M>"],
+           4: ["k_hc2_contract_fma<M>", "k_hc2_sum<M>"]}
 
 
 def time_mode(sp, mcb, torch, T, V, dCs, dHCs, mode, steps, warmup, barrier):
@@ -293,7 +295,7 @@ def run_gpu(args):
     timed_build(mcb.FOCK_TABLE, "fock_table")            # second build = warm timing
     mode = MODES[args.mode]
     if mode == 0:
-        mode = mcb.GEMM if c.N >= 2 else mcb.REHASH
+        mode = mcb.REHASH if c.N < 2 else (mcb.FMA if 2 <= c.M <= 6 else mcb.GEMM)     # what MCB_AUTO resolves to
     map_bytes = 0
     if mode == mcb.MAPS:
         timed_build(mcb.MAP1, "map1")
@@ -341,7 +343,7 @@ def run_gpu(args):
                     "algorithmic_bytes_per_launch": alg_bytes}
     else:
         # contract kernel (GEMM mode) carries every two-body term + the folded one-body terms: 8 flop per packed term
-        kflops = 8.0 * tc["two_body_terms_packed"] if mode == mcb.GEMM else flops_step
+        kflops = 8.0 * tc["two_body_terms_packed"] if mode in (mcb.GEMM, mcb.FMA) else flops_step
         roofline = {"bound": "alu", "kernel": KERNELS[mode][dom], "achieved": kflops / (dom_ms * 1e-3) / 1e12,
                     "peak": alu_peak, "unit": "TFLOP/s",
                     "peak_source": f"derived: 148 SM x 64 DFMA/clk x 2 x {peaks['sm_max_mhz']:.0f} MHz (DESIGN.md)",
@@ -357,7 +359,7 @@ def run_gpu(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "complex128 (f64)", "data": "synthetic (seeded, workloads.py)",
-        "config": dict(config_dict(c, {1: "MAPS", 2: "REHASH", 3: "GEMM"}[mode]),
+        "config": dict(config_dict(c, MODE_NAMES[mode]),
                        l2="inputs larger than L2: 3 rotating C and 3 rotating HC buffers, 16*nc bytes each",
                        replicas="N>1 = independent replicas (path does not shard by north_star)"),
         "applications_per_s": world / (ms_step * 1e-3),
@@ -374,8 +376,8 @@ def run_gpu(args):
     # ---- the other variants, short (map-memory vs recompute trade-off) ----
     if args.variants and rank == 0 and world == 1:
         var = {}
-        for name, m in (("REHASH", mcb.REHASH), ("GEMM", mcb.GEMM), ("MAPS", mcb.MAPS)):
-            if m == mode or (m == mcb.GEMM and c.N < 2):
+        for name, m in (("REHASH", mcb.REHASH), ("GEMM", mcb.GEMM), ("FMA", mcb.FMA), ("MAPS", mcb.MAPS)):
+            if m == mode or (m in (mcb.GEMM, mcb.FMA) and c.N < 2) or (m == mcb.FMA and not 2 <= c.M <= 6):
                 continue
             try:
                 if m == mcb.MAPS:
