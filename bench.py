@@ -234,10 +234,10 @@ class Job:
 # ------------------------------------------------------------------------------------------------------------
 # GPU arm
 # ------------------------------------------------------------------------------------------------------------
-MODES = {"auto": 0, "maps": 1, "rehash": 2, "gemm": 3, "fma": 4}
-MODE_NAMES = {1: "MAPS", 2: "REHASH", 3: "GEMM", 4: "FMA"}
+MODES = {"auto": 0, "maps": 1, "rehash": 2, "gemm": 3, "runs": 4}
+MODE_NAMES = {1: "MAPS", 2: "REHASH", 3: "GEMM", 4: "RUNS"}
 KERNELS = {1: ["k_hc_direct<M,maps>"], 2: ["k_hc_direct<M,rehash>"], 3: ["k_hc2_contract<M>", "k_hc2_reduce<M>"],
-           4: ["k_hc2_contract_fma<M>", "k_hc2_sum<M>"]}
+           4: ["k_hc2_contract_runs<M>", "k_hc2_sum<M>"]}
 
 
 def time_mode(sp, mcb, torch, T, V, dCs, dHCs, mode, steps, warmup, barrier):
@@ -295,7 +295,7 @@ def run_gpu(args):
     timed_build(mcb.FOCK_TABLE, "fock_table")            # second build = warm timing
     mode = MODES[args.mode]
     if mode == 0:
-        mode = mcb.REHASH if c.N < 2 else (mcb.FMA if 2 <= c.M <= 6 else mcb.GEMM)     # what MCB_AUTO resolves to
+        mode = mcb.REHASH if c.N < 2 else (mcb.RUNS if 2 <= c.M <= 5 else mcb.GEMM)     # what MCB_AUTO resolves to
     map_bytes = 0
     if mode == mcb.MAPS:
         timed_build(mcb.MAP1, "map1")
@@ -343,7 +343,7 @@ def run_gpu(args):
                     "algorithmic_bytes_per_launch": alg_bytes}
     else:
         # contract kernel (GEMM mode) carries every two-body term + the folded one-body terms: 8 flop per packed term
-        kflops = 8.0 * tc["two_body_terms_packed"] if mode in (mcb.GEMM, mcb.FMA) else flops_step
+        kflops = 8.0 * tc["two_body_terms_packed"] if mode in (mcb.GEMM, mcb.RUNS) else flops_step
         roofline = {"bound": "alu", "kernel": KERNELS[mode][dom], "achieved": kflops / (dom_ms * 1e-3) / 1e12,
                     "peak": alu_peak, "unit": "TFLOP/s",
                     "peak_source": f"derived: 148 SM x 64 DFMA/clk x 2 x {peaks['sm_max_mhz']:.0f} MHz (DESIGN.md)",
@@ -376,8 +376,8 @@ def run_gpu(args):
     # ---- the other variants, short (map-memory vs recompute trade-off) ----
     if args.variants and rank == 0 and world == 1:
         var = {}
-        for name, m in (("REHASH", mcb.REHASH), ("GEMM", mcb.GEMM), ("FMA", mcb.FMA), ("MAPS", mcb.MAPS)):
-            if m == mode or (m in (mcb.GEMM, mcb.FMA) and c.N < 2) or (m == mcb.FMA and not 2 <= c.M <= 6):
+        for name, m in (("REHASH", mcb.REHASH), ("GEMM", mcb.GEMM), ("RUNS", mcb.RUNS), ("MAPS", mcb.MAPS)):
+            if m == mode or (m in (mcb.GEMM, mcb.RUNS) and c.N < 2) or (m == mcb.RUNS and not 2 <= c.M <= 5):
                 continue
             try:
                 if m == mcb.MAPS:

@@ -45,7 +45,7 @@ extern "C" {
 
 #define MCB_MAX_M        32   /* hashing and map kernels                                                      */
 #define MCB_MAX_M_APPLY  12   /* hc_apply: packed V (P x P complex, P = M(M+1)/2) must fit on chip            */
-#define MCB_MAX_M_FMA     6   /* MCB_FMA: the P gathered values of an intermediate must fit in registers      */
+#define MCB_MAX_M_RUNS    5   /* MCB_RUNS: the embedded coefficient matrix must fit in register fragments      */
 
 /* structures that live in caller-provided device memory (mcb_structure_bytes / mcb_build_structure) */
 #define MCB_FOCK_TABLE    0   /* "hashing table" of all occupation vectors, for the N- and
@@ -54,7 +54,7 @@ extern "C" {
 #define MCB_MAP2          2   /* double-jump map, dense [pair(k<=s)][pair(q<=l)][b] layout  */
 
 /* hc_apply modes */
-#define MCB_AUTO          0   /* N < 2: MCB_REHASH; 2 <= M <= MCB_MAX_M_FMA: MCB_FMA; else MCB_GEMM                */
+#define MCB_AUTO          0   /* N < 2: MCB_REHASH; 2 <= M <= MCB_MAX_M_RUNS: MCB_RUNS; else MCB_GEMM              */
 #define MCB_MAPS          1   /* per-output gather through the stored Map1 + Map2 (the paper's fastest CPU/GPU
                                  variant); needs FOCK_TABLE, MAP1, MAP2                      */
 #define MCB_REHASH        2   /* per-output gather, target indices recomputed on the fly from the hashing table
@@ -62,11 +62,12 @@ extern "C" {
 #define MCB_GEMM          3   /* on-the-fly rehashing, two-body term factored through the (N-2)-particle space:
                                  W = Vpacked . (F * C[jump]) as an FP64 tensor-core contraction, then a gather;
                                  T folded into V via sum_s a+_s a_s = N.  needs FOCK_TABLE and a workspace     */
-#define MCB_FMA           4   /* the same factorisation for few orbitals (2 <= M <= MCB_MAX_M_FMA, N >= 2; the
-                                 paper's "M = 3..5, N up to 1000" shape): one thread per
-                                 (N-2)-particle intermediate on the plain FP64 pipe, contributions that stay
-                                 inside a run of the index order pre-summed, then a streaming sum over
-                                 output-indexed planes.  needs FOCK_TABLE and a workspace                     */
+#define MCB_RUNS          4   /* the same factorisation for few orbitals (2 <= M <= MCB_MAX_M_RUNS, N >= 2; the
+                                 paper's "M = 3..5, N up to 1000" shape): every warp walks a
+                                 segment of consecutive (N-2)-particle intermediates (asynchronous gathers, FP64
+                                 tensor-core contraction), contributions that stay inside a run of the index
+                                 order are pre-summed, then a streaming sum over output-indexed planes.
+                                 needs FOCK_TABLE and a workspace                                             */
 
 typedef struct mcb_space mcb_space;          /* opaque */
 typedef struct { double re, im; } mcb_c128;

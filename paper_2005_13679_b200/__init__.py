@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libmcb.so")
 
 OK, EINVAL, ERANGE, ENOMEM, ECUDA, ENOTREADY, EUNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
 FOCK_TABLE, MAP1, MAP2 = 0, 1, 2
-AUTO, MAPS, REHASH, GEMM, FMA = 0, 1, 2, 3, 4
+AUTO, MAPS, REHASH, GEMM, RUNS = 0, 1, 2, 3, 4
 MAX_M, MAX_M_APPLY = 32, 12
 
 EXPORTS = (

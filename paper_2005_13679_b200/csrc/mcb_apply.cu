@@ -205,8 +205,8 @@ __global__ void __launch_bounds__(128) k_hc_direct(DirectArgs p)
 
 static int resolve_mode(const mcb_space* sp, int mode)
 {
-    if (mode == MCB_AUTO) return sp->N < 2 ? MCB_REHASH : (mcb_fma_supported(sp) ? MCB_FMA : MCB_GEMM);
-    if ((mode == MCB_GEMM || mode == MCB_FMA) && sp->N < 2) return MCB_REHASH;   // no (N-2)-particle space: one-body only
+    if (mode == MCB_AUTO) return sp->N < 2 ? MCB_REHASH : (mcb_runs_supported(sp) ? MCB_RUNS : MCB_GEMM);
+    if ((mode == MCB_GEMM || mode == MCB_RUNS) && sp->N < 2) return MCB_REHASH;   // no (N-2)-particle space: one-body only
     return mode;
 }
 
@@ -214,9 +214,9 @@ extern "C" long long mcb_apply_workspace_bytes(const mcb_space* sp, int mode)
 {
     if (!sp) return MCB_EINVAL;
     if (sp->M > MCB_MAX_M_APPLY) return MCB_EUNSUPPORTED;
-    if (mode < MCB_AUTO || mode > MCB_FMA) return MCB_EINVAL;
+    if (mode < MCB_AUTO || mode > MCB_RUNS) return MCB_EINVAL;
     mode = resolve_mode(sp, mode);
-    if (mode == MCB_FMA) return mcb_fma_supported(sp) ? mcb_fma_workspace_bytes(sp) : (long long)MCB_EUNSUPPORTED;
+    if (mode == MCB_RUNS) return mcb_runs_supported(sp) ? mcb_runs_workspace_bytes(sp) : (long long)MCB_EUNSUPPORTED;
     if (mode != MCB_GEMM) return 0;
     return mcb_gemm_workspace_bytes(sp);
 }
@@ -262,7 +262,7 @@ extern "C" int mcb_hc_apply(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
                             const mcb_c128* d_C, mcb_c128* d_HC, int mode, void* d_workspace, void* stream)
 {
     if (!sp || !T || !V || !d_C || !d_HC) return MCB_EINVAL;
-    if (mode < MCB_AUTO || mode > MCB_FMA) return MCB_EINVAL;
+    if (mode < MCB_AUTO || mode > MCB_RUNS) return MCB_EINVAL;
     if (sp->M > MCB_MAX_M_APPLY) return MCB_EUNSUPPORTED;
     if ((((uintptr_t)d_C) & 15) || (((uintptr_t)d_HC) & 15)) return MCB_EINVAL;
     {
@@ -274,10 +274,10 @@ extern "C" int mcb_hc_apply(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
     mode = resolve_mode(sp, mode);
     cudaStream_t st = (cudaStream_t)stream;
     if (mode == MCB_MAPS && (!sp->d_map1 || (sp->N >= 2 && !sp->d_map2))) return MCB_ENOTREADY;
-    if (mode == MCB_FMA) {
-        if (!mcb_fma_supported(sp)) return MCB_EUNSUPPORTED;
+    if (mode == MCB_RUNS) {
+        if (!mcb_runs_supported(sp)) return MCB_EUNSUPPORTED;
         if (!d_workspace || (((uintptr_t)d_workspace) & 255)) return MCB_EINVAL;
-        return mcb_launch_fma(sp, T, V, d_C, d_HC, d_workspace, st);
+        return mcb_launch_runs(sp, T, V, d_C, d_HC, d_workspace, st);
     } else if (mode == MCB_GEMM) {
         if (!d_workspace || (((uintptr_t)d_workspace) & 255)) return MCB_EINVAL;
         return mcb_launch_gemm(sp, T, V, d_C, d_HC, d_workspace, st);

@@ -1,0 +1,419 @@
+// mcb_apply_runs.cu -- MCB_RUNS mode of hc_apply (Eq. 12-13) for few orbitals (2 <= M <= 5).
+//
+// Same factorisation through the (N-2)-particle space as MCB_GEMM (mcb_apply_gemm.cu),
+//     H = sum_m sum_{a=(k<=s)} sum_{c=(q<=l)} |m+e_k+e_s> F(m,a) Vp[a][c] F(m,c) <m+e_q+e_l|   (T folded into Vp),
+// laid out for the "few orbitals, many particles" shape (M = 3..5, N = 100..1000), where the
+// index order has long runs (only n_0, n_1 change inside a run; run length ~ (N+M-1)/(M-1)):
+//
+//   k_hc2_contract_runs<M>: every WARP owns a segment of consecutive intermediates and walks it in chunks of 32,
+//     software-pipelined three deep:
+//       A  (lane = intermediate)  occupations of chunk ch+2 are loaded; for chunk ch+1 the index arithmetic
+//          (mcb_device.cuh) runs and the P targets of C are gathered with cp.async straight into the warp's
+//          shared-memory stage Z[c][m]; the factors F(m,c) and the output indices go beside them;
+//       B  (tensor path)          for chunk ch, four 8-intermediate blocks: A-fragment = F(m,c) * Z[c][m] read from
+//          the stage, B-fragment = the packed coefficients embedded as a real (2P x 2P) matrix, STATIONARY in
+//          registers; mma.sync.m8n8k4.f64 (SASS DMMA) accumulates W'[a][m], which is scaled by F(m,a) and staged
+//          in shared memory;
+//       C  (lane = intermediate)  in-run pre-summation and store.  Orbitals 0 and 1 only move a configuration
+//          inside its run (index +-1), so the removal pairs fall into classes kappa = (the part of e_k+e_s on
+//          orbitals >= 2):
+//              {}      : (0,0) (0,1) (1,1)          -> outputs g0, g0+1, g0+2 with g0 = index(m + 2 e_0)
+//              {h}     : (0,h) (1,h)                -> outputs gh, gh+1       with gh = index(m + e_0 + e_h)
+//              {h,h'}  : (h,h')                     -> output  index(m + e_h + e_h')
+//          and the contributions of one class to one output come from up to three NEIGHBOURING intermediates of
+//          the same run -- neighbouring slots of the stage.  They are summed and written once into a plane
+//          Hp[kappa][g] indexed by the OUTPUT configuration (NCLS = 1 + (M-2) + (M-2)(M-1)/2 planes instead of
+//          P), each (kappa, g) slot by exactly one thread: no atomics.
+//   k_hc2_sum<M>: HC[g] = sum over the classes allowed at g of Hp[kappa][g] -- a coalesced stream.
+#include <string.h>
+#include "mcb_device.cuh"
+
+__host__ __device__ constexpr int rdiv(int a, int b) { return (a + b - 1) / b; }
+
+template <int M> struct RunCfg {
+    static constexpr int P = M * (M + 1) / 2;
+    static constexpr int NH = M - 2;                               // orbitals that leave the run
+    static constexpr int NCLS = 1 + NH + NH * (NH + 1) / 2;        // classes = planes
+    static constexpr int NK = rdiv(2 * P, 4);                      // k-steps (contraction over (c, re|im))
+    static constexpr int NB = rdiv(2 * P, 8);                      // 8-column blocks of outputs (a, re|im)
+    static constexpr int CHUNKS = 32;                              // 32-wide chunks per warp segment
+    static constexpr int SEG = CHUNKS * 32 - 2;                    // intermediates OWNED per segment (2 halo lanes)
+    // per-warp shared memory, two stages of
+    //   [2 carry slots][ Z / W' : P rows x ZLD double2 ][ F : P rows x FLD double ][ META : MROWS rows x 32 int ]
+    // Z[c][m] receives the gathered C values of chunk ch; once the DMMAs of the chunk are done the same rows hold
+    // W'[a][m] for phase C.  Slots 32..35 of a row are padding (36 % 8 == 4 makes the A-fragment reads conflict
+    // free); slots 34, 35 of row a - 1 (the two slots in FRONT of row a) carry W'[a] of lanes 30, 31 of the
+    // previous chunk -- cp.async never touches them, so they are written into the stage that is being filled.
+    static constexpr int ZLD = 36;
+    static constexpr int FLD = 40;                                 // doubles per row of F
+    static constexpr int MROWS = NCLS + 1;                         // int rows of META: output index per class, flags
+    static constexpr int STAGES = 2;
+    static constexpr size_t HEAD_BYTES = 32;
+    static constexpr size_t Z_BYTES = (size_t)P * ZLD * 16;
+    static constexpr size_t F_BYTES = (size_t)P * FLD * 8;
+    static constexpr size_t META_BYTES = (size_t)MROWS * 32 * 4;
+    static constexpr size_t STAGE_BYTES = HEAD_BYTES + Z_BYTES + F_BYTES + META_BYTES;
+    static constexpr size_t WARP_BYTES = STAGES * STAGE_BYTES;
+    // warps per CTA / CTAs per SM: as many warps as the 227 KB hold, in two CTAs
+    static constexpr int WARPS_SM = (int)((227 * 1024 - 2 * 1024) / WARP_BYTES);
+    static constexpr int WARPS = WARPS_SM / 2 > 8 ? 8 : WARPS_SM / 2;
+    static constexpr int THREADS = WARPS * 32;
+    static constexpr size_t SMEM = WARPS * WARP_BYTES;
+    static constexpr int MINB = 2;
+    static_assert(STAGE_BYTES % 16 == 0 && Z_BYTES % 16 == 0 && F_BYTES % 16 == 0, "alignment");
+    static_assert(WARPS >= 1, "shared memory");
+};
+
+// Coefficient matrix of the embedded real product, B[kappa][n] with kappa = 2 c + (re|im of the gathered value),
+// n = 2 a + (re|im of the result):   W.re = sum Vr z.re - Vi z.im,   W.im = sum Vi z.re + Vr z.im
+template <int M> struct RunCoef { double b[RunCfg<M>::NK * 4][RunCfg<M>::NB * 8]; };     // T folded in, zero padded
+
+struct RunArgs {
+    McbDev d;
+    McbFockView fock;
+    const double2* C;
+    double2* HC;
+    double2* Hp;               // [NCLS][ldp]
+    long long ldp;
+    int nseg;                  // warp segments
+};
+
+__device__ __forceinline__ int run_cls_single(int h) { return 1 + (h - 2); }
+template <int M> __device__ __forceinline__ constexpr int run_cls_pair(int h, int h2)
+{
+    // pair index over the NH high orbitals, (h-2) <= (h2-2)
+    return 1 + (M - 2) + mcb_pair_index(M - 2, h - 2, h2 - 2);
+}
+
+__device__ __forceinline__ void run_dmma884(double& c0, double& c1, const double a, const double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+// ---- cp.async (LDGSTS): 16-byte global -> shared copies that do not hold a register while in flight ----------
+__device__ __forceinline__ void cp_async16(double2* smem_dst, const double2* gsrc, bool valid)
+{
+    const unsigned dst = (unsigned)__cvta_generic_to_shared(smem_dst);
+    const int bytes = valid ? 16 : 0;                                   // 0 -> the slot is zero-filled
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(gsrc), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// occupations of intermediate m from the hashing table (zeros outside [0, nc2))
+template <int M>
+__device__ __forceinline__ void run_load_occ(const RunArgs& p, const int m, int (&occ)[M])
+{
+    const bool valid = m >= 0 && m < p.d.nc2;
+#pragma unroll
+    for (int j = 0; j < M; ++j) occ[j] = valid ? (int)__ldg(p.fock.occ2 + (long long)j * p.fock.ld2 + m) : 0;
+}
+
+// Phase A for one intermediate (this lane's slot of the stage): index arithmetic, asynchronous gather of the P
+// targets of C, factors F(m,c) = sqrt((m_q+1)(m_l+1+[q==l])), output indices and flags.
+template <int M>
+__device__ __forceinline__ void run_prefetch(const RunArgs& p, const int m, const int (&occ)[M], const int seg0, const int seg_end,
+                                             unsigned char* __restrict__ stage, const int lane)
+{
+    using Cfg = RunCfg<M>;
+    constexpr int P = Cfg::P;
+    const McbDev& d = p.d;
+    double2* const Z = reinterpret_cast<double2*>(stage + Cfg::HEAD_BYTES) + lane;
+    double* const F = reinterpret_cast<double*>(stage + Cfg::HEAD_BYTES + Cfg::Z_BYTES) + lane;
+    int* const META = reinterpret_cast<int*>(stage + Cfg::HEAD_BYTES + Cfg::Z_BYTES + Cfg::F_BYTES) + lane;
+    const bool valid = m >= 0 && m < d.nc2;
+    const bool own = valid && m >= seg0 && m < seg_end;
+    int X[M], Y[M], mj0 = 0, mj1 = 0;
+    double r1[M], r2[M];
+    {
+        int A1[M], A2[M];
+        int run = 0, x = 0, tot1 = 0;
+#pragma unroll
+        for (int j = 0; j < M; ++j) {
+            const int nj = occ[j];
+            if (j == 0) mj0 = nj;
+            if (j == 1) mj1 = nj;
+            run += nj;
+            r1[j] = __ldg(d.sq + nj + 1);
+            r2[j] = __ldg(d.sq2 + nj + 2);
+            X[j] = x;
+            if (j == 0) {
+                // G[0][s] = binom(s, 1) = s: no look-up
+                A1[0] = run + 1; A2[0] = run + 2;
+                x += -1; tot1 += A1[0];
+            } else if (j <= M - 2) {
+                const int a0 = mcb_ldG(d.G, d.ldg, j, run);
+                A1[j] = mcb_ldG(d.G, d.ldg, j, run + 1);
+                A2[j] = mcb_ldG(d.G, d.ldg, j, run + 2);
+                x += a0 - A1[j]; tot1 += A1[j];
+            } else { A1[j] = 0; A2[j] = 0; }
+        }
+        int pre = tot1, suf = 0;
+#pragma unroll
+        for (int l = M - 1; l >= 0; --l) { pre -= A1[l]; suf += A2[l]; Y[l] = pre + suf; }
+    }
+    const int base = d.nc - 1;
+    {
+        int c = 0;
+#pragma unroll
+        for (int q = 0; q < M; ++q) {
+#pragma unroll
+            for (int l = q; l < M; ++l, ++c) {
+                cp_async16(Z + c * Cfg::ZLD, p.C + (valid ? base - X[q] - Y[l] : 0), valid);
+                F[c * Cfg::FLD] = (q == l) ? r2[q] : r1[q] * r1[l];
+            }
+        }
+    }
+    META[0] = base - X[0] - Y[0];
+#pragma unroll
+    for (int h = 2; h < M; ++h) {
+        META[run_cls_single(h) * 32] = base - X[0] - Y[h];
+#pragma unroll
+        for (int h2 = h; h2 < M; ++h2) META[run_cls_pair<M>(h, h2) * 32] = base - X[h] - Y[h2];
+    }
+    META[Cfg::NCLS * 32] = (own ? 1 : 0) | (mj0 == 0 ? 2 : 0) | (mj1 << 2);
+}
+
+__device__ __forceinline__ void cadd(double2& o, const double2 w) { o.x += w.x; o.y += w.y; }
+
+template <int M>
+__global__ void __launch_bounds__(RunCfg<M>::THREADS, RunCfg<M>::MINB)
+k_hc2_contract_runs(const RunArgs p, const __grid_constant__ RunCoef<M> coef)
+{
+    using Cfg = RunCfg<M>;
+    constexpr int P = Cfg::P, NK = Cfg::NK, NB = Cfg::NB;
+    extern __shared__ __align__(16) unsigned char run_smem[];
+    const McbDev& d = p.d;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int grp = lane >> 2, tig = lane & 3;
+    const int seg = blockIdx.x * Cfg::WARPS + warp;
+    if (seg >= p.nseg) return;
+    const int seg0 = seg * Cfg::SEG;
+    const int seg_end = min(seg0 + Cfg::SEG, d.nc2);
+    const int first = seg0 - 2;                                          // two halo lanes in front of the segment
+    const int nch = (seg_end - first + 31) >> 5;                         // warp-uniform, <= CHUNKS
+    unsigned char* const wbase = run_smem + (size_t)warp * Cfg::WARP_BYTES;
+
+    // stationary B-fragments: b[ks][nb] = B[4 ks + tig][8 nb + grp]
+    double bfrag[NK][NB];
+#pragma unroll
+    for (int ks = 0; ks < NK; ++ks)
+#pragma unroll
+        for (int nb = 0; nb < NB; ++nb) bfrag[ks][nb] = coef.b[4 * ks + tig][8 * nb + grp];
+
+    int occ[M];
+    run_load_occ<M>(p, first + lane, occ);
+    run_prefetch<M>(p, first + lane, occ, seg0, seg_end, wbase, lane);
+    cp_async_commit();
+    if (1 < nch) run_load_occ<M>(p, first + 32 + lane, occ);
+
+#pragma unroll 1
+    for (int ch = 0; ch < nch; ++ch) {
+        // ---- phase A: chunk ch + 1 (gathers fly under the DMMAs of chunk ch), occupations of chunk ch + 2 ----
+        unsigned char* const stage_next = wbase + ((ch + 1) & 1) * Cfg::STAGE_BYTES;
+        if (ch + 1 < nch)
+            run_prefetch<M>(p, first + (ch + 1) * 32 + lane, occ, seg0, seg_end, stage_next, lane);
+        cp_async_commit();
+        if (ch + 2 < nch) run_load_occ<M>(p, first + (ch + 2) * 32 + lane, occ);
+        cp_async_wait<1>();                                              // this lane's gathers of chunk ch have landed
+        __syncwarp();                                                    // ... and everybody else's
+        unsigned char* const stage = wbase + (ch & 1) * Cfg::STAGE_BYTES;
+        const double* Zd = reinterpret_cast<const double*>(stage + Cfg::HEAD_BYTES);                          // [P][ZLD][re|im]
+        double2* const W = reinterpret_cast<double2*>(stage + Cfg::HEAD_BYTES);                               // [P][ZLD], after the DMMAs
+        const double* F = reinterpret_cast<const double*>(stage + Cfg::HEAD_BYTES + Cfg::Z_BYTES);             // [P][FLD]
+        const int* META = reinterpret_cast<const int*>(stage + Cfg::HEAD_BYTES + Cfg::Z_BYTES + Cfg::F_BYTES); // [MROWS][32]
+
+        // ---- phase B: W'[a][m] = F(m,a) sum_c Vp[a][c] F(m,c) Z[c][m]; the four 8-intermediate blocks of the
+        //      chunk are in flight together: 4 NB independent DMMA accumulator chains ----
+        {
+            double acc[4][NB][2];
+#pragma unroll
+            for (int cb = 0; cb < 4; ++cb)
+#pragma unroll
+                for (int nb = 0; nb < NB; ++nb) { acc[cb][nb][0] = 0.0; acc[cb][nb][1] = 0.0; }
+#pragma unroll
+            for (int ks = 0; ks < NK; ++ks) {
+                const int c = 2 * ks + (tig >> 1);                       // kappa = 4 ks + tig = 2 c + part
+                double a[4];
+#pragma unroll
+                for (int cb = 0; cb < 4; ++cb) {
+                    a[cb] = 0.0;
+                    if (2 * ks + 1 < P || c < P)
+                        a[cb] = Zd[(c * Cfg::ZLD + cb * 8 + grp) * 2 + (tig & 1)] * F[c * Cfg::FLD + cb * 8 + grp];
+                }
+#pragma unroll
+                for (int cb = 0; cb < 4; ++cb)
+#pragma unroll
+                    for (int nb = 0; nb < NB; ++nb) run_dmma884(acc[cb][nb][0], acc[cb][nb][1], a[cb], bfrag[ks][nb]);
+            }
+            __syncwarp();                                                // every lane is done with Z: the rows become W'
+#pragma unroll
+            for (int cb = 0; cb < 4; ++cb)
+#pragma unroll
+                for (int nb = 0; nb < NB; ++nb) {
+                    const int ar = 4 * nb + tig;                         // this lane holds (re, im) of W'[ar][cb * 8 + grp]
+                    if (4 * nb + 3 < P || ar < P) {
+                        const double f = F[ar * Cfg::FLD + cb * 8 + grp];
+                        W[ar * Cfg::ZLD + cb * 8 + grp] = make_double2(f * acc[cb][nb][0], f * acc[cb][nb][1]);
+                    }
+                }
+        }
+        __syncwarp();
+
+        // ---- phase C: in-run pre-summation (lane = intermediate; slots -1, -2 of lane 0 are the carry slots) and
+        //      one store per (class, output) ----
+        {
+            const double2* Wl = W + lane;
+            const int flags = META[Cfg::NCLS * 32 + lane];
+            const bool own = flags & 1, last = flags & 2;
+            const int mj1 = flags >> 2;
+            constexpr int a00 = mcb_pair_index(M, 0, 0), a01 = mcb_pair_index(M, 0, 1), a11 = mcb_pair_index(M, 1, 1);
+            if (own) {
+                // class {}: pairs (0,0), (0,1), (1,1)
+                double2 o = Wl[a00 * Cfg::ZLD];
+                if (mj1 >= 1) cadd(o, Wl[a01 * Cfg::ZLD - 1]);
+                if (mj1 >= 2) cadd(o, Wl[a11 * Cfg::ZLD - 2]);
+                double2* dst = p.Hp + META[lane];
+                __stcg(dst, o);
+                if (last) {
+                    double2 e = Wl[a01 * Cfg::ZLD];
+                    if (mj1 >= 1) cadd(e, Wl[a11 * Cfg::ZLD - 1]);
+                    __stcg(dst + 1, e);
+                    __stcg(dst + 2, Wl[a11 * Cfg::ZLD]);
+                }
+                // class {h}: pairs (0,h), (1,h)
+#pragma unroll
+                for (int h = 2; h < M; ++h) {
+                    const int a0 = mcb_pair_index(M, 0, h), a1 = mcb_pair_index(M, 1, h);
+                    double2 oh = Wl[a0 * Cfg::ZLD];
+                    if (mj1 >= 1) cadd(oh, Wl[a1 * Cfg::ZLD - 1]);
+                    double2* dh = p.Hp + (long long)run_cls_single(h) * p.ldp + META[run_cls_single(h) * 32 + lane];
+                    __stcg(dh, oh);
+                    if (last) __stcg(dh + 1, Wl[a1 * Cfg::ZLD]);
+                }
+                // class {h,h'}: one pair, one output
+#pragma unroll
+                for (int h = 2; h < M; ++h) {
+#pragma unroll
+                    for (int h2 = h; h2 < M; ++h2) {
+                        const int cls = run_cls_pair<M>(h, h2);
+                        __stcg(p.Hp + (long long)cls * p.ldp + META[cls * 32 + lane], Wl[mcb_pair_index(M, h, h2) * Cfg::ZLD]);
+                    }
+                }
+            }
+            if (lane >= 30) {                                            // carry the rows that neighbours read
+                double2* Wn = reinterpret_cast<double2*>(stage_next + Cfg::HEAD_BYTES) + lane - 32;
+                Wn[a01 * Cfg::ZLD] = Wl[a01 * Cfg::ZLD];
+                Wn[a11 * Cfg::ZLD] = Wl[a11 * Cfg::ZLD];
+#pragma unroll
+                for (int h = 2; h < M; ++h) Wn[mcb_pair_index(M, 1, h) * Cfg::ZLD] = Wl[mcb_pair_index(M, 1, h) * Cfg::ZLD];
+            }
+            __syncwarp();                                                // W' of this stage may now be overwritten
+        }
+    }
+}
+
+// HC[g] = sum over the classes allowed at g of Hp[kappa][g]
+template <int M>
+__global__ void __launch_bounds__(256) k_hc2_sum(const RunArgs p)
+{
+    const McbDev& d = p.d;
+    const int g = blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= d.nc) return;
+    int n[M];
+#pragma unroll
+    for (int j = 0; j < M; ++j) n[j] = p.fock.occ[(long long)j * p.fock.ld + g];
+    const int in01 = n[0] + n[1];
+    const double2* src = p.Hp + g;
+    double re = 0.0, im = 0.0;
+    if (in01 >= 2) { const double2 w = __ldcs(src); re += w.x; im += w.y; }
+#pragma unroll
+    for (int h = 2; h < M; ++h) {
+        if (n[h] >= 1 && in01 >= 1) {
+            const double2 w = __ldcs(src + (long long)run_cls_single(h) * p.ldp);
+            re += w.x; im += w.y;
+        }
+    }
+#pragma unroll
+    for (int h = 2; h < M; ++h) {
+#pragma unroll
+        for (int h2 = h; h2 < M; ++h2) {
+            const bool ok = (h == h2) ? (n[h] >= 2) : (n[h] >= 1 && n[h2] >= 1);
+            if (ok) {
+                const double2 w = __ldcs(src + (long long)run_cls_pair<M>(h, h2) * p.ldp);
+                re += w.x; im += w.y;
+            }
+        }
+    }
+    p.HC[g] = make_double2(re, im);
+}
+
+// =========================================================================================================
+// host
+// =========================================================================================================
+static long long runs_ldp(const mcb_space* sp) { return mcb_round_up(sp->nc, 128); }
+
+bool mcb_runs_supported(const mcb_space* sp) { return sp->M >= 2 && sp->M <= MCB_MAX_M_RUNS && sp->N >= 2; }
+
+long long mcb_runs_workspace_bytes(const mcb_space* sp)
+{
+    const int NH = sp->M - 2;
+    const int ncls = 1 + NH + NH * (NH + 1) / 2;
+    return (long long)ncls * runs_ldp(sp) * (long long)sizeof(double2);
+}
+
+template <int M>
+static int launch_runs(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
+                       const mcb_c128* d_C, mcb_c128* d_HC, void* d_ws, cudaStream_t st)
+{
+    using Cfg = RunCfg<M>;
+    constexpr int P = Cfg::P;
+    double* vr = (double*)sp->h_coef;
+    double* vi = vr + P * P;
+    if ((char*)(vi + P * P) > (char*)sp->h_coef + sp->coef_bytes) return MCB_ENOMEM;
+    mcb_pack_pairs(sp->N, M, T, V, true, vr, vi);
+    static RunCoef<M> coef;                                              // too large for the stack at M = 6
+    memset(&coef, 0, sizeof(coef));
+    for (int a = 0; a < P; ++a)
+        for (int c = 0; c < P; ++c) {
+            const double re = vr[a * P + c], im = vi[a * P + c];
+            coef.b[2 * c][2 * a] = re;       coef.b[2 * c + 1][2 * a] = -im;
+            coef.b[2 * c][2 * a + 1] = im;   coef.b[2 * c + 1][2 * a + 1] = re;
+        }
+
+    RunArgs a;
+    a.d = sp->dev; a.fock = sp->fock;
+    a.C = (const double2*)d_C; a.HC = (double2*)d_HC;
+    a.Hp = (double2*)d_ws; a.ldp = runs_ldp(sp);
+    a.nseg = (int)((sp->nc2 + Cfg::SEG - 1) / Cfg::SEG);
+    const unsigned grid = (unsigned)((a.nseg + Cfg::WARPS - 1) / Cfg::WARPS);
+    static bool attr_set = false;
+    if (!attr_set) {
+        MCB_CUDA(cudaFuncSetAttribute(k_hc2_contract_runs<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
+        attr_set = true;
+    }
+    { int rc = mcb_tick(sp, 0, st); if (rc) return rc; }
+    k_hc2_contract_runs<M><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(a, coef);
+    MCB_CHECK_LAUNCH();
+    { int rc = mcb_tick(sp, 1, st); if (rc) return rc; }
+    const int threads = 256;
+    k_hc2_sum<M><<<(unsigned)((sp->nc + threads - 1) / threads), threads, 0, st>>>(a);
+    MCB_CHECK_LAUNCH();
+    { int rc = mcb_tick(sp, 2, st); if (rc) return rc; }
+    mcb_tick_done(sp, 2);
+    sp->last_launches = 2;
+    return MCB_OK;
+}
+
+int mcb_launch_runs(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, const mcb_c128* d_C, mcb_c128* d_HC,
+                    void* d_ws, cudaStream_t st)
+{
+    switch (sp->M) {
+    case 2: return launch_runs<2>(sp, T, V, d_C, d_HC, d_ws, st);
+    case 3: return launch_runs<3>(sp, T, V, d_C, d_HC, d_ws, st);
+    case 4: return launch_runs<4>(sp, T, V, d_C, d_HC, d_ws, st);
+    case 5: return launch_runs<5>(sp, T, V, d_C, d_HC, d_ws, st);
+    default: return MCB_EUNSUPPORTED;
+    }
+}

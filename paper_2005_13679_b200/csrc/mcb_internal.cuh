@@ -75,10 +75,10 @@ long long mcb_gemm_workspace_bytes(const mcb_space* sp);
 int mcb_launch_gemm(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, const mcb_c128* d_C, mcb_c128* d_HC,
                     void* d_ws, cudaStream_t st);
 
-// MCB_FMA mode (mcb_apply_fma.cu)
-bool mcb_fma_supported(const mcb_space* sp);
-long long mcb_fma_workspace_bytes(const mcb_space* sp);
-int mcb_launch_fma(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, const mcb_c128* d_C, mcb_c128* d_HC,
+// MCB_RUNS mode (mcb_apply_runs.cu)
+bool mcb_runs_supported(const mcb_space* sp);
+long long mcb_runs_workspace_bytes(const mcb_space* sp);
+int mcb_launch_runs(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, const mcb_c128* d_C, mcb_c128* d_HC,
                    void* d_ws, cudaStream_t st);
 
 // measurement support (mcb_timing_enable): event i of the current apply's slot, recorded on the apply's stream

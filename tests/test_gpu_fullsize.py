@@ -48,8 +48,8 @@ def test_hc_apply_sampled_rows_all_modes(mcb, cfg):
     ref, _ = oracle.hc_apply(c.N, c.M, T, V, C, rows=rows)
     dC = torch.from_numpy(C).cuda()
     modes = [("GEMM", mcb.GEMM), ("REHASH", mcb.REHASH)]
-    if 2 <= c.M <= 6:
-        modes.append(("FMA", mcb.FMA))
+    if 2 <= c.M <= 5:
+        modes.append(("RUNS", mcb.RUNS))
     if _maps_fit(sp, mcb):
         sp.build_structure(mcb.MAP1)
         sp.build_structure(mcb.MAP2)
@@ -91,7 +91,7 @@ def test_hermiticity_and_constant_interaction_full_size(mcb, cfg):
             Vc[k, s, k, s] = U
     T0 = np.zeros((M, M), dtype=np.complex128)
     expect = U * c.N * (c.N - 1) / 2
-    for mode in (mcb.GEMM, mcb.REHASH) + ((mcb.FMA,) if 2 <= M <= 6 else ()):
+    for mode in (mcb.GEMM, mcb.REHASH) + ((mcb.RUNS,) if 2 <= M <= 5 else ()):
         out = sp.hc_apply(T0, Vc, du, mode=mode)
         err = float((out - expect * du).abs().max())
         assert err <= 1e-12 * abs(U) * c.N * c.N * np.abs(u).max() * 4, (mode, err)

@@ -94,12 +94,12 @@ def test_structures_small(mcb, N, M):
 
 
 @pytest.mark.parametrize("N,M", SMALL)
-@pytest.mark.parametrize("mode", ["REHASH", "MAPS", "GEMM", "FMA"])
+@pytest.mark.parametrize("mode", ["REHASH", "MAPS", "GEMM", "RUNS"])
 def test_hc_apply_small(mcb, N, M, mode):
     if mode == "MAPS" and M > 8:
         pytest.skip("Map2 not built for large M in the small-case sweep")
-    if mode == "FMA" and not (2 <= M <= 6 and N >= 2):
-        pytest.skip("MCB_FMA covers 2 <= M <= 6, N >= 2")
+    if mode == "RUNS" and not (2 <= M <= 5 and N >= 2):
+        pytest.skip("MCB_RUNS covers 2 <= M <= 5, N >= 2")
     sp = mcb.Space(N, M)
     nc = sp.nc
     T, V, C = workloads.make_small_inputs(N, M, nc, seed=1000 + 17 * N + M, general_V=(N + M) % 2 == 0)
