@@ -237,7 +237,7 @@ class Job:
 MODES = {"auto": 0, "maps": 1, "rehash": 2, "gemm": 3, "runs": 4}
 MODE_NAMES = {1: "MAPS", 2: "REHASH", 3: "GEMM", 4: "RUNS"}
 KERNELS = {1: ["k_hc_direct<M,maps>"], 2: ["k_hc_direct<M,rehash>"], 3: ["k_hc2_contract<M>", "k_hc2_reduce<M>"],
-           4: ["k_hc2_contract_runs<M>", "k_hc2_sum<M>"]}
+           4: ["k_hc2_runs<M>"]}
 
 
 def time_mode(sp, mcb, torch, T, V, dCs, dHCs, mode, steps, warmup, barrier):

@@ -28,6 +28,9 @@
 #include <string.h>
 #include "mcb_device.cuh"
 
+#ifndef RUNS_CHUNKS
+#define RUNS_CHUNKS 16
+#endif
 __host__ __device__ constexpr int rdiv(int a, int b) { return (a + b - 1) / b; }
 
 template <int M> struct RunCfg {
@@ -36,7 +39,7 @@ template <int M> struct RunCfg {
     static constexpr int NCLS = 1 + NH + NH * (NH + 1) / 2;        // classes = planes
     static constexpr int NK = rdiv(2 * P, 4);                      // k-steps (contraction over (c, re|im))
     static constexpr int NB = rdiv(2 * P, 8);                      // 8-column blocks of outputs (a, re|im)
-    static constexpr int CHUNKS = 32;                              // 32-wide chunks per warp segment
+    static constexpr int CHUNKS = RUNS_CHUNKS;                              // 32-wide chunks per segment (one ticket)
     static constexpr int SEG = CHUNKS * 32 - 2;                    // intermediates OWNED per segment (2 halo lanes)
     // per-warp shared memory, two stages of
     //   [2 carry slots][ Z / W' : P rows x ZLD double2 ][ F : P rows x FLD double ][ META : MROWS rows x 32 int ]
@@ -57,7 +60,9 @@ template <int M> struct RunCfg {
     // warps per CTA / CTAs per SM: as many warps as the 227 KB hold, in two CTAs
     static constexpr int WARPS_SM = (int)((227 * 1024 - 2 * 1024) / WARP_BYTES);
     static constexpr int WARPS = WARPS_SM / 2 > 8 ? 8 : WARPS_SM / 2;
-    static constexpr int THREADS = WARPS * 32;
+    static constexpr int THREADS = (WARPS + 1) * 32;               // + one warp per CTA that only sums
+    static constexpr int SUM_TILE = 512;                           // outputs per sum ticket
+    static constexpr int SUM_U = (NCLS <= 6) ? 4 : 2;                  // outputs in flight per lane
     static constexpr size_t SMEM = WARPS * WARP_BYTES;
     static constexpr int MINB = 2;
     static_assert(STAGE_BYTES % 16 == 0 && Z_BYTES % 16 == 0 && F_BYTES % 16 == 0, "alignment");
@@ -75,7 +80,10 @@ struct RunArgs {
     double2* HC;
     double2* Hp;               // [NCLS][ldp]
     long long ldp;
-    int nseg;                  // warp segments
+    int nseg;                  // warp segments of the contraction
+    int ntile;                 // output tiles of the sum (SUM_TILE outputs each)
+    int* flags;                // [nseg] segment s has been contracted and its class planes are visible
+    int* tickets;              // [4] next segment, next output tile, verified prefix of flags, pad (zeroed with the flags)
 };
 
 __device__ __forceinline__ int run_cls_single(int h) { return 1 + (h - 2); }
@@ -177,9 +185,101 @@ __device__ __forceinline__ void run_prefetch(const RunArgs& p, const int m, cons
 
 __device__ __forceinline__ void cadd(double2& o, const double2 w) { o.x += w.x; o.y += w.y; }
 
+__device__ __forceinline__ int run_ticket(int* ctr, const int lane)
+{
+    int t = 0;
+    if (lane == 0) t = atomicAdd(ctr, 1);
+    return __shfl_sync(0xffffffffu, t, 0);
+}
+
+// HC[g] = sum over the classes allowed at g of Hp[kappa][g], for output tiles taken in index order.  A tile whose
+// largest top occupation n_{M-1} is j needs every intermediate with m_{M-1} <= j, a PREFIX of the intermediate
+// order (nc2 - N_c(N-3-j, M) of them): the warp waits until the segments of that prefix are flagged.  The
+// contraction never waits for anything, so this cannot deadlock; it trails the contraction closely enough for
+// the class planes to be read from L2.
+template <int M>
+__device__ __forceinline__ void run_sum_tiles(const RunArgs& p, const int lane)
+{
+    using Cfg = RunCfg<M>;
+    const McbDev& d = p.d;
+    int wm = 0;                                                          // segments < wm are known to be done
+    for (;;) {
+        const int t = run_ticket(p.tickets + 1, lane);
+        if (t >= p.ntile) break;
+        const int g0 = t * Cfg::SUM_TILE;
+        const int g1 = min(g0 + Cfg::SUM_TILE, d.nc);
+        const int jmax = (int)__ldg(p.fock.occ + (long long)(M - 1) * p.fock.ld + (g1 - 1));
+        const int tt = max(d.N - 2 - jmax, 0);
+        const int need_int = d.nc2 - mcb_ldG(d.G, d.ldg, M - 2, tt);     // G[M-2][t] = N_c(t - 1, M)
+        const int need_seg = (need_int + Cfg::SEG - 1) / Cfg::SEG;
+        if (wm < need_seg) {
+            wm = max(wm, *reinterpret_cast<volatile int*>(p.tickets + 2));          // what other warps have verified
+            const int wm_in = wm;
+            while (wm < need_seg) {
+                // probe 128 flags per round trip; indices outside [wm, need_seg) count as set
+                const int a = wm & ~127;
+                const int4 f4 = __ldcv(reinterpret_cast<const int4*>(p.flags + a) + lane);
+                const int f[4] = {f4.x, f4.y, f4.z, f4.w};
+                int first_unset = 4;
+#pragma unroll
+                for (int i = 3; i >= 0; --i) {
+                    const int idx = a + 4 * lane + i;
+                    if (idx >= wm && idx < need_seg && f[i] == 0) first_unset = i;
+                }
+                const unsigned ball = __ballot_sync(0xffffffffu, first_unset < 4);
+                if (ball == 0u) wm = a + 128;
+                else {
+                    const int src = __ffs(ball) - 1;
+                    wm = a + 4 * src + __shfl_sync(0xffffffffu, first_unset, src);
+                    __nanosleep(500);
+                }
+            }
+            wm = min(wm, need_seg);
+            if (lane == 0 && wm > wm_in) atomicMax(p.tickets + 2, wm);
+        }
+        __threadfence();
+#pragma unroll 1
+        for (int gb = g0; gb < g1; gb += 32 * Cfg::SUM_U) {
+            // all loads of SUM_U outputs are issued before the first add: SUM_U * NCLS 16-byte loads in flight per lane
+            double2 w[Cfg::SUM_U][Cfg::NCLS];
+#pragma unroll
+            for (int u = 0; u < Cfg::SUM_U; ++u) {
+                const int g = gb + u * 32 + lane;
+                const bool live = g < g1;
+                int n[M];
+#pragma unroll
+                for (int j = 0; j < M; ++j) n[j] = live ? (int)__ldg(p.fock.occ + (long long)j * p.fock.ld + g) : 0;
+                const int in01 = n[0] + n[1];
+                const double2* src = p.Hp + g;
+                const double2 zero = make_double2(0.0, 0.0);
+                w[u][0] = (in01 >= 2) ? __ldcg(src) : zero;
+#pragma unroll
+                for (int h = 2; h < M; ++h)
+                    w[u][run_cls_single(h)] = (n[h] >= 1 && in01 >= 1) ? __ldcg(src + (long long)run_cls_single(h) * p.ldp) : zero;
+#pragma unroll
+                for (int h = 2; h < M; ++h) {
+#pragma unroll
+                    for (int h2 = h; h2 < M; ++h2) {
+                        const bool ok = (h == h2) ? (n[h] >= 2) : (n[h] >= 1 && n[h2] >= 1);
+                        w[u][run_cls_pair<M>(h, h2)] = ok ? __ldcg(src + (long long)run_cls_pair<M>(h, h2) * p.ldp) : zero;
+                    }
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < Cfg::SUM_U; ++u) {
+                const int g = gb + u * 32 + lane;
+                double re = 0.0, im = 0.0;
+#pragma unroll
+                for (int k = 0; k < Cfg::NCLS; ++k) { re += w[u][k].x; im += w[u][k].y; }
+                if (g < g1) __stcs(p.HC + g, make_double2(re, im));
+            }
+        }
+    }
+}
+
 template <int M>
 __global__ void __launch_bounds__(RunCfg<M>::THREADS, RunCfg<M>::MINB)
-k_hc2_contract_runs(const RunArgs p, const __grid_constant__ RunCoef<M> coef)
+k_hc2_runs(const RunArgs p, const __grid_constant__ RunCoef<M> coef)
 {
     using Cfg = RunCfg<M>;
     constexpr int P = Cfg::P, NK = Cfg::NK, NB = Cfg::NB;
@@ -187,12 +287,7 @@ k_hc2_contract_runs(const RunArgs p, const __grid_constant__ RunCoef<M> coef)
     const McbDev& d = p.d;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int grp = lane >> 2, tig = lane & 3;
-    const int seg = blockIdx.x * Cfg::WARPS + warp;
-    if (seg >= p.nseg) return;
-    const int seg0 = seg * Cfg::SEG;
-    const int seg_end = min(seg0 + Cfg::SEG, d.nc2);
-    const int first = seg0 - 2;                                          // two halo lanes in front of the segment
-    const int nch = (seg_end - first + 31) >> 5;                         // warp-uniform, <= CHUNKS
+    if (warp == Cfg::WARPS) { run_sum_tiles<M>(p, lane); return; }       // the summing warp of this CTA
     unsigned char* const wbase = run_smem + (size_t)warp * Cfg::WARP_BYTES;
 
     // stationary B-fragments: b[ks][nb] = B[4 ks + tig][8 nb + grp]
@@ -202,23 +297,49 @@ k_hc2_contract_runs(const RunArgs p, const __grid_constant__ RunCoef<M> coef)
 #pragma unroll
         for (int nb = 0; nb < NB; ++nb) bfrag[ks][nb] = coef.b[4 * ks + tig][8 * nb + grp];
 
+    // The warp walks a STREAM of chunks: the chunks of one short segment after the other, segments taken in index
+    // order from a global ticket, so that at any moment all warps of the GPU work inside a narrow window of the
+    // intermediate order (the class planes they write are still in L2 when the sum reads them) while the software
+    // pipeline (occupations of chunk i+2 | gathers of chunk i+1 | DMMAs of chunk i) never drains.
+    struct Chunk { int m0, seg0, seg_end, seg; bool valid, last; };
+    int gen_seg = 0, gen_ch = 0, gen_nch = 0;                            // generator state: next chunk of the stream
+    auto next_chunk = [&](Chunk& c) {
+        if (gen_ch == gen_nch) {                                         // segment exhausted: take the next ticket
+            gen_seg = run_ticket(p.tickets, lane);
+            gen_ch = 0;
+            gen_nch = gen_seg < p.nseg ? (min(gen_seg * Cfg::SEG + Cfg::SEG, d.nc2) - (gen_seg * Cfg::SEG - 2) + 31) >> 5 : 0;
+            if (gen_nch == 0) { gen_nch = -1; }                          // no work left, stay exhausted
+        }
+        c.valid = gen_nch > 0;
+        if (!c.valid) { gen_ch = gen_nch = -1; c.m0 = 0; c.seg0 = 0; c.seg_end = 0; c.seg = 0; c.last = false; return; }
+        c.seg = gen_seg;
+        c.seg0 = gen_seg * Cfg::SEG;
+        c.seg_end = min(c.seg0 + Cfg::SEG, d.nc2);
+        c.m0 = c.seg0 - 2 + gen_ch * 32;                                 // two halo lanes in front of the segment
+        ++gen_ch;
+        c.last = gen_ch == gen_nch;
+    };
+    Chunk c0, c1, c2;
+    next_chunk(c0); next_chunk(c1); next_chunk(c2);
     int occ[M];
-    run_load_occ<M>(p, first + lane, occ);
-    run_prefetch<M>(p, first + lane, occ, seg0, seg_end, wbase, lane);
+    int st = 0;
+    if (c0.valid) {
+        run_load_occ<M>(p, c0.m0 + lane, occ);
+        run_prefetch<M>(p, c0.m0 + lane, occ, c0.seg0, c0.seg_end, wbase, lane);
+    }
     cp_async_commit();
-    if (1 < nch) run_load_occ<M>(p, first + 32 + lane, occ);
+    if (c1.valid) run_load_occ<M>(p, c1.m0 + lane, occ);
 
 #pragma unroll 1
-    for (int ch = 0; ch < nch; ++ch) {
-        // ---- phase A: chunk ch + 1 (gathers fly under the DMMAs of chunk ch), occupations of chunk ch + 2 ----
-        unsigned char* const stage_next = wbase + ((ch + 1) & 1) * Cfg::STAGE_BYTES;
-        if (ch + 1 < nch)
-            run_prefetch<M>(p, first + (ch + 1) * 32 + lane, occ, seg0, seg_end, stage_next, lane);
+    while (c0.valid) {
+        // ---- phase A: next chunk (its gathers fly under the DMMAs of this one), occupations of the one after ----
+        unsigned char* const stage_next = wbase + (st ^ 1) * Cfg::STAGE_BYTES;
+        if (c1.valid) run_prefetch<M>(p, c1.m0 + lane, occ, c1.seg0, c1.seg_end, stage_next, lane);
         cp_async_commit();
-        if (ch + 2 < nch) run_load_occ<M>(p, first + (ch + 2) * 32 + lane, occ);
+        if (c2.valid) run_load_occ<M>(p, c2.m0 + lane, occ);
         cp_async_wait<1>();                                              // this lane's gathers of chunk ch have landed
         __syncwarp();                                                    // ... and everybody else's
-        unsigned char* const stage = wbase + (ch & 1) * Cfg::STAGE_BYTES;
+        unsigned char* const stage = wbase + st * Cfg::STAGE_BYTES;
         const double* Zd = reinterpret_cast<const double*>(stage + Cfg::HEAD_BYTES);                          // [P][ZLD][re|im]
         double2* const W = reinterpret_cast<double2*>(stage + Cfg::HEAD_BYTES);                               // [P][ZLD], after the DMMAs
         const double* F = reinterpret_cast<const double*>(stage + Cfg::HEAD_BYTES + Cfg::Z_BYTES);             // [P][FLD]
@@ -311,48 +432,27 @@ k_hc2_contract_runs(const RunArgs p, const __grid_constant__ RunCoef<M> coef)
             }
             __syncwarp();                                                // W' of this stage may now be overwritten
         }
-    }
-}
-
-// HC[g] = sum over the classes allowed at g of Hp[kappa][g]
-template <int M>
-__global__ void __launch_bounds__(256) k_hc2_sum(const RunArgs p)
-{
-    const McbDev& d = p.d;
-    const int g = blockIdx.x * blockDim.x + threadIdx.x;
-    if (g >= d.nc) return;
-    int n[M];
-#pragma unroll
-    for (int j = 0; j < M; ++j) n[j] = p.fock.occ[(long long)j * p.fock.ld + g];
-    const int in01 = n[0] + n[1];
-    const double2* src = p.Hp + g;
-    double re = 0.0, im = 0.0;
-    if (in01 >= 2) { const double2 w = __ldcs(src); re += w.x; im += w.y; }
-#pragma unroll
-    for (int h = 2; h < M; ++h) {
-        if (n[h] >= 1 && in01 >= 1) {
-            const double2 w = __ldcs(src + (long long)run_cls_single(h) * p.ldp);
-            re += w.x; im += w.y;
+        if (c0.last) {                                                   // publish: the class-plane stores of the segment
+            __syncwarp();                                                // are visible before its flag: the barrier orders
+            if (lane == 0)                                               // the warp's stores before lane 0's release store
+                asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p.flags + c0.seg), "r"(1) : "memory");
         }
+        c0 = c1; c1 = c2; next_chunk(c2);
+        st ^= 1;
     }
-#pragma unroll
-    for (int h = 2; h < M; ++h) {
-#pragma unroll
-        for (int h2 = h; h2 < M; ++h2) {
-            const bool ok = (h == h2) ? (n[h] >= 2) : (n[h] >= 1 && n[h2] >= 1);
-            if (ok) {
-                const double2 w = __ldcs(src + (long long)run_cls_pair<M>(h, h2) * p.ldp);
-                re += w.x; im += w.y;
-            }
-        }
-    }
-    p.HC[g] = make_double2(re, im);
+    run_sum_tiles<M>(p, lane);                                           // no segment left: help with the sum
 }
 
 // =========================================================================================================
 // host
 // =========================================================================================================
 static long long runs_ldp(const mcb_space* sp) { return mcb_round_up(sp->nc, 128); }
+// tickets [2] + segment flags; sized for the shortest segment any M uses
+static long long runs_sync_bytes(const mcb_space* sp)
+{
+    const long long nseg = (sp->nc2 + RunCfg<2>::SEG - 1) / RunCfg<2>::SEG;
+    return mcb_round_up((mcb_round_up(nseg, 128) + 4) * (long long)sizeof(int), 256);
+}
 
 bool mcb_runs_supported(const mcb_space* sp) { return sp->M >= 2 && sp->M <= MCB_MAX_M_RUNS && sp->N >= 2; }
 
@@ -360,7 +460,7 @@ long long mcb_runs_workspace_bytes(const mcb_space* sp)
 {
     const int NH = sp->M - 2;
     const int ncls = 1 + NH + NH * (NH + 1) / 2;
-    return (long long)ncls * runs_ldp(sp) * (long long)sizeof(double2);
+    return (long long)ncls * runs_ldp(sp) * (long long)sizeof(double2) + runs_sync_bytes(sp);
 }
 
 template <int M>
@@ -387,22 +487,29 @@ static int launch_runs(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
     a.C = (const double2*)d_C; a.HC = (double2*)d_HC;
     a.Hp = (double2*)d_ws; a.ldp = runs_ldp(sp);
     a.nseg = (int)((sp->nc2 + Cfg::SEG - 1) / Cfg::SEG);
-    const unsigned grid = (unsigned)((a.nseg + Cfg::WARPS - 1) / Cfg::WARPS);
-    static bool attr_set = false;
-    if (!attr_set) {
-        MCB_CUDA(cudaFuncSetAttribute(k_hc2_contract_runs<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
-        attr_set = true;
+    a.ntile = (int)((sp->nc + Cfg::SUM_TILE - 1) / Cfg::SUM_TILE);
+    {
+        const int NH = M - 2;
+        const long long planes = (long long)(1 + NH + NH * (NH + 1) / 2) * a.ldp * (long long)sizeof(double2);
+        a.tickets = reinterpret_cast<int*>((char*)d_ws + planes);
+        a.flags = a.tickets + 4;
+    }
+    static int grid = 0;
+    if (!grid) {
+        int per_sm = 0, sms = 0;
+        MCB_CUDA(cudaFuncSetAttribute(k_hc2_runs<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
+        MCB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_hc2_runs<M>, Cfg::THREADS, Cfg::SMEM));
+        MCB_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, sp->device));
+        if (per_sm < 1) return MCB_EUNSUPPORTED;
+        grid = per_sm * sms;
     }
     { int rc = mcb_tick(sp, 0, st); if (rc) return rc; }
-    k_hc2_contract_runs<M><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(a, coef);
+    MCB_CUDA(cudaMemsetAsync(a.tickets, 0, (size_t)(mcb_round_up(a.nseg, 128) + 4) * sizeof(int), st));
+    k_hc2_runs<M><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(a, coef);
     MCB_CHECK_LAUNCH();
     { int rc = mcb_tick(sp, 1, st); if (rc) return rc; }
-    const int threads = 256;
-    k_hc2_sum<M><<<(unsigned)((sp->nc + threads - 1) / threads), threads, 0, st>>>(a);
-    MCB_CHECK_LAUNCH();
-    { int rc = mcb_tick(sp, 2, st); if (rc) return rc; }
-    mcb_tick_done(sp, 2);
-    sp->last_launches = 2;
+    mcb_tick_done(sp, 1);
+    sp->last_launches = 1;
     return MCB_OK;
 }
 
