@@ -240,6 +240,15 @@ KERNELS = {1: ["k_hc_direct<M,maps>"], 2: ["k_hc_direct<M,rehash>"], 3: ["k_hc2_
            4: ["k_hc2_runs<M>"]}
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the committed `ncu --set full`
+# captures (profiles/*.md name the commands); None where no capture of the current kernel exists.
+NCU_TRAFFIC_BYTES = {
+    (2, 4): (1.410871e9 + 1.194112e9, "profiles/r1_cfg2_runs_v5.md"),
+    (1, 4): (0.879559e9 + 0.763621e9, "profiles/r1_cfg2_runs_v5.md"),
+    (4, 3): (0.448114e9 + 3.060399e9, "profiles/r1_cfg4_gemm_v1.md"),
+}
+
+
 def time_mode(sp, mcb, torch, T, V, dCs, dHCs, mode, steps, warmup, barrier):
     """Device time of `steps` applies (CUDA events on the launching stream), plus per-kernel times."""
     R = len(dCs)
@@ -348,6 +357,9 @@ def run_gpu(args):
                     "peak": alu_peak, "unit": "TFLOP/s",
                     "peak_source": f"derived: 148 SM x 64 DFMA/clk x 2 x {peaks['sm_max_mhz']:.0f} MHz (DESIGN.md)",
                     "traffic": None, "algorithmic_flops_per_launch": kflops}
+    if (args.cfg, mode) in NCU_TRAFFIC_BYTES:
+        roofline["traffic"], roofline["traffic_source"] = NCU_TRAFFIC_BYTES[(args.cfg, mode)]
+        roofline["traffic_unit"] = "bytes per launch (dram read + write, one ncu --set full capture)"
     roofline["frac"] = roofline["achieved"] / roofline["peak"]
     roofline["kernel_ms"] = dom_ms
     roofline["kernel_share_of_step"] = dom_ms / ms_step
