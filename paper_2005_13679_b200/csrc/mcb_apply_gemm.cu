@@ -23,7 +23,8 @@ __host__ __device__ constexpr int cdiv(int a, int b) { return (a + b - 1) / b; }
 //   EMBED (small M): the complex P x P product is embedded as a real 2P x 2P one with rows ordered (a, re|im):
 //        row 2a   = [ Vr[a][:] | -Vi[a][:] ],  row 2a+1 = [ Vi[a][:] | Vr[a][:] ],  D rows = [ Dr ; Di ],
 //        which pads 2P (not P) to the 8 x 4 fragment grid;
-//   otherwise: real fragments of Vr, Vi and three accumulators (Vr.Dr, Vi.Di, Vr.Di + Vi.Dr).
+//   otherwise: real fragments of Vr, Vi and three accumulators Vr.Dr, Vi.Di, (Vr + Vi).(Dr + Di): the complex
+//        product with three real multiplications (re = t0 - t1, im = t2 - t0 - t1).
 // Consumer warp (wr, wc) owns row blocks {wr, wr + WR, ..} (8 rows each) for ALL k-steps and sweeps the column
 // blocks (8 intermediates each) {2 wc, 2 wc + 1, 2 wc + 2 WC, ..} of the tile.
 template <int M> struct GemmCfg {
@@ -254,20 +255,21 @@ __global__ void __launch_bounds__(GemmCfg<M>::THREADS, GemmCfg<M>::MINB) k_hc2_c
                 const double br0 = b_base[ks * 4 * LD], br1 = b_base[ks * 4 * LD + 8];
                 double bi0 = 0.0, bi1 = 0.0;
                 if (!EMBED) { bi0 = b_base[Cfg::DROWS * LD + ks * 4 * LD]; bi1 = b_base[Cfg::DROWS * LD + ks * 4 * LD + 8]; }
+                const double bs0 = br0 + bi0, bs1 = br1 + bi1;
 #pragma unroll
                 for (int i = 0; i < NRB; ++i) {
                     if (EMBED) {
                         dmma884(acc[i][0][0][0], acc[i][0][0][1], a_re[i][ks], br0);
                         dmma884(acc[i][1][0][0], acc[i][1][0][1], a_re[i][ks], br1);
                     } else {
+                        // complex product with three real ones: Vr.Dr, Vi.Di, (Vr + Vi).(Dr + Di)   (reading A19)
+                        const double a_s = a_re[i][ks] + a_im[i][ks];
                         dmma884(acc[i][0][0][0], acc[i][0][0][1], a_re[i][ks], br0);
                         dmma884(acc[i][1][0][0], acc[i][1][0][1], a_re[i][ks], br1);
                         dmma884(acc[i][0][1][0], acc[i][0][1][1], a_im[i][ks], bi0);
                         dmma884(acc[i][1][1][0], acc[i][1][1][1], a_im[i][ks], bi1);
-                        dmma884(acc[i][0][2][0], acc[i][0][2][1], a_re[i][ks], bi0);
-                        dmma884(acc[i][1][2][0], acc[i][1][2][1], a_re[i][ks], bi1);
-                        dmma884(acc[i][0][2][0], acc[i][0][2][1], a_im[i][ks], br0);
-                        dmma884(acc[i][1][2][0], acc[i][1][2][1], a_im[i][ks], br1);
+                        dmma884(acc[i][0][2][0], acc[i][0][2][1], a_s, bs0);
+                        dmma884(acc[i][1][2][0], acc[i][1][2][1], a_s, bs1);
                     }
                 }
             }
@@ -297,8 +299,8 @@ __global__ void __launch_bounds__(GemmCfg<M>::THREADS, GemmCfg<M>::MINB) k_hc2_c
                         if (k == sI) { f0 = R2[k * TM + col]; f1 = R2[k * TM + col + 1]; }
                         else { f0 = R1[k * TM + col] * R1[sI * TM + col]; f1 = R1[k * TM + col + 1] * R1[sI * TM + col + 1]; }
                         double2* w = p.W + (size_t)mcb_pair_index(M, k, sI) * p.ldw + m0 + col;
-                        w[0] = make_double2(f0 * (acc[i][j][0][0] - acc[i][j][1][0]), f0 * acc[i][j][2][0]);
-                        w[1] = make_double2(f1 * (acc[i][j][0][1] - acc[i][j][1][1]), f1 * acc[i][j][2][1]);
+                        w[0] = make_double2(f0 * (acc[i][j][0][0] - acc[i][j][1][0]), f0 * ((acc[i][j][2][0] - acc[i][j][0][0]) - acc[i][j][1][0]));
+                        w[1] = make_double2(f1 * (acc[i][j][0][1] - acc[i][j][1][1]), f1 * ((acc[i][j][2][1] - acc[i][j][0][1]) - acc[i][j][1][1]));
                     }
                 }
             }
