@@ -337,19 +337,38 @@ __global__ void __launch_bounds__(256) k_hc2_reduce(GemmArgs p)
 #pragma unroll
         for (int l = M - 1; l >= 0; --l) { pre -= A1[l]; suf += A2[l]; Y[l] = pre + suf; }
     }
+    // the allowed W' elements are fetched in batches of RB_ loads that are all in flight before the first add
+    // (latency-bound gather: run length of the index order is only ~(N+M-1)/(M-1))
+    constexpr int P = M * (M + 1) / 2;
+#ifndef REDUCE_BATCH
+#define REDUCE_BATCH 16
+#endif
+    constexpr int RB_ = P <= REDUCE_BATCH ? P : REDUCE_BATCH;
     double re = 0.0, im = 0.0;
-    int a = 0;
+    int mi[P];
+    bool ok[P];
+    {
+        int a = 0;
 #pragma unroll
-    for (int k = 0; k < M; ++k) {
+        for (int k = 0; k < M; ++k) {
 #pragma unroll
-        for (int s = k; s < M; ++s, ++a) {
-            const bool ok = (k == s) ? (n[k] >= 2) : (n[k] >= 1 && n[s] >= 1);
-            if (ok) {
-                const int mi = d.nc2 - 1 - X[k] - Y[s];
-                const double2 w = __ldg(p.W + (size_t)a * p.ldw + mi);
-                re += w.x; im += w.y;
+            for (int s = k; s < M; ++s, ++a) {
+                ok[a] = (k == s) ? (n[k] >= 2) : (n[k] >= 1 && n[s] >= 1);
+                mi[a] = d.nc2 - 1 - X[k] - Y[s];
             }
         }
+    }
+#pragma unroll
+    for (int a0 = 0; a0 < P; a0 += RB_) {
+        double2 w[RB_];
+#pragma unroll
+        for (int i = 0; i < RB_; ++i) {
+            const int a = a0 + i;
+            w[i] = make_double2(0.0, 0.0);
+            if (a < P && ok[a]) w[i] = __ldcs(p.W + (size_t)a * p.ldw + mi[a]);
+        }
+#pragma unroll
+        for (int i = 0; i < RB_; ++i) { re += w[i].x; im += w[i].y; }
     }
     p.HC[g] = make_double2(re, im);
 }
