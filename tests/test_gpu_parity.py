@@ -112,3 +112,40 @@ def test_hc_apply_small(mcb, N, M, mode):
     err = np.abs(got - ref).max()
     assert err <= tol(T, V, C), (err, tol(T, V, C))
     sp.close()
+
+
+# MCB_RUNS is one persistent kernel: warps take 510-intermediate segments by ticket and a trailing role sums the class
+# planes behind per-segment flags.  These spaces span many segments and CTAs with ragged tails (nc2 not a multiple
+# of 32 or of the segment), runs shorter and longer than a warp, and the smallest (N-2)-particle spaces (nc2 = 1).
+RUNS_SPACES = [(2, 2), (2, 3), (2, 5), (3, 2), (3, 5), (4, 4), (60, 4), (30, 5), (200, 3), (2000, 2), (33, 4), (17, 5)]
+
+
+@pytest.mark.parametrize("N,M", RUNS_SPACES)
+def test_hc_apply_runs_many_segments(mcb, N, M):
+    sp = mcb.Space(N, M)
+    nc = sp.nc
+    T, V, C = workloads.make_small_inputs(N, M, nc, seed=4242 + 31 * N + M, general_V=(N + M) % 2 == 1)
+    ref, _ = oracle.hc_apply(N, M, T, V, C)
+    sp.build_structure(mcb.FOCK_TABLE)
+    dC = torch.from_numpy(C).cuda()
+    got = sp.hc_apply(T, V, dC, mode=mcb.RUNS)
+    err = np.abs(got.cpu().numpy() - ref).max()
+    # The north-star bound 1e-12 * ||T,V||max * ||C||_1 does not grow with the amplitudes (up to N^2): at N = 2000 it is
+    # 5 ulp of the largest |HC| (~1e5), tighter than ANY reordering of an fp64 sum of 2 P^2 terms can promise.  Beyond
+    # the paper's range (N <= 1000) the bound is the arithmetic one of DESIGN.md section 2: 64 ulp of max|HC|.
+    t = max(tol(T, V, C), 64 * 2.0 ** -53 * np.abs(ref).max()) if N > 1000 else tol(T, V, C)
+    assert err <= t, (err, t)
+    assert sp.last_apply_launches() == 1
+    # the workspace (class planes, tickets, flags) is reused: a second apply, on a side stream, gives the same bits
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        again = sp.hc_apply(T, V, dC, mode=mcb.RUNS, stream=side)
+    side.synchronize()
+    a, b = got.cpu().numpy(), again.cpu().numpy()
+    assert (a == b).all()        # no atomics, fixed summation order: bit-identical
+    # AUTO resolves to RUNS here and must agree with the per-output REHASH path
+    auto = sp.hc_apply(T, V, dC, mode=mcb.AUTO).cpu().numpy()
+    rehash = sp.hc_apply(T, V, dC, mode=mcb.REHASH).cpu().numpy()
+    assert np.abs(auto - ref).max() <= t and np.abs(rehash - ref).max() <= t
+    sp.close()
