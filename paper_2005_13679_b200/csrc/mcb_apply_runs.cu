@@ -5,8 +5,9 @@
 // laid out for the "few orbitals, many particles" shape (M = 3..5, N = 100..1000), where the
 // index order has long runs (only n_0, n_1 change inside a run; run length ~ (N+M-1)/(M-1)):
 //
-//   k_hc2_contract_runs<M>: every WARP owns a segment of consecutive intermediates and walks it in chunks of 32,
-//     software-pipelined three deep:
+// ONE persistent kernel per apply, k_hc2_runs<M>, with two roles.
+//   CONTRACTING warps take short segments of consecutive intermediates in index order from a global ticket and walk
+//     them in chunks of 32, as one software pipeline that never drains, three deep:
 //       A  (lane = intermediate)  occupations of chunk ch+2 are loaded; for chunk ch+1 the index arithmetic
 //          (mcb_device.cuh) runs and the P targets of C are gathered with cp.async straight into the warp's
 //          shared-memory stage Z[c][m]; the factors F(m,c) and the output indices go beside them;
@@ -24,7 +25,9 @@
 //          the same run -- neighbouring slots of the stage.  They are summed and written once into a plane
 //          Hp[kappa][g] indexed by the OUTPUT configuration (NCLS = 1 + (M-2) + (M-2)(M-1)/2 planes instead of
 //          P), each (kappa, g) slot by exactly one thread: no atomics.
-//   k_hc2_sum<M>: HC[g] = sum over the classes allowed at g of Hp[kappa][g] -- a coalesced stream.
+//   SUMMING warps (one per CTA, and every contracting warp once the tickets run out) take tiles of outputs in index
+//     order: HC[g] = sum over the classes allowed at g of Hp[kappa][g], a coalesced stream that trails the
+//     contraction behind per-segment release/acquire flags (run_sum_tiles).
 #include <string.h>
 #include "mcb_device.cuh"
 
