@@ -41,6 +41,8 @@ def lib():
         L.mcbo_hc_apply_rows.argtypes = [i, i, p, p, p, p, ll, p, i]
         L.mcbo_hc_apply_rows.restype = i
         L.mcbo_max_threads.restype = i
+        L.mcbo_rho.argtypes = [i, i, p, p, p]
+        L.mcbo_rho.restype = None
         _lib = L
     return _lib
 
@@ -109,6 +111,15 @@ def hc_apply(N: int, M: int, T: np.ndarray, V: np.ndarray, C: np.ndarray,
     out = np.empty(nrows, dtype=np.complex128)
     used = lib().mcbo_hc_apply_rows(N, M, _ptr(T), _ptr(V), _ptr(C), rp, nrows, _ptr(out), nthreads)
     return out, used
+
+
+def rho(N: int, M: int, C: np.ndarray):
+    """(rho1 [M,M], rho2 [M,M,M,M]) complex128: <a+_k a_l>, <a+_k a+_s a_q a_l> (Eq. 10, 11; App. B index order)."""
+    C = np.ascontiguousarray(C, dtype=np.complex128).reshape(-1)
+    r1 = np.empty((M, M), dtype=np.complex128)
+    r2 = np.empty((M, M, M, M), dtype=np.complex128)
+    lib().mcbo_rho(N, M, _ptr(C), _ptr(r1), _ptr(r2))
+    return r1, r2
 
 
 def max_threads() -> int:

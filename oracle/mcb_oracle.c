@@ -14,6 +14,8 @@
  *   mcbo_map2          double-jump map  Map2[b][(k<=s)][(q<=l)]          PAPER.md:206-224   (reading A15)
  *   mcbo_hc_apply_rows HC_g = sum_b <n^g|H|n^b> C_b for a list of rows g Eq. (3),(4),(12),(13) PAPER.md:49-53,101-107
  *                      H = sum T_kl a+_k a_l + 1/2 sum V_ksql a+_k a+_s a_q a_l (north star; reading A6)
+ *   mcbo_rho           rho1[k][l] = <Psi|a+_k a_l|Psi>, rho2[k][s][q][l] = <Psi|a+_k a+_s a_q a_l|Psi>
+ *                      Eq. (10),(11) PAPER.md:93-97; index order of App. B PAPER.md:377 (reading A11)
  *
  * The apply is the plain definition: for each output row g the ORDERED sums over (k,l) and
  * (k,s,q,l) are written out, each target index recomputed with the literal O(N) Algorithm 1
@@ -232,6 +234,57 @@ int mcbo_hc_apply_rows(int N, int M, const zc *T, const zc *V, const zc *C,
     }
     free(tab);
     return used;
+}
+
+/* ---- Eq. (10), (11): one- and two-body density matrices ---------------------------------------------------
+ *  rho1[k*M+l] = sum_{g,b} conj(C_g) C_b <n^g| a+_k a_l |n^b>,
+ *  rho2[((k*M+s)*M+q)*M+l] = sum_{g,b} conj(C_g) C_b <n^g| a+_k a+_s a_q a_l |n^b>   (App. B labels rho_ksql),
+ *  written out as the double sum: for every bra g and every ordered index tuple the single ket b with a non-zero
+ *  element is found by the literal Algorithm 1, amplitudes as in mcbo_hc_apply_rows (ladder algebra, Eq. 1, 5).
+ *  Serial, one accumulation order.  With these conventions <Psi|H|Psi> = sum T_kl rho1_kl + 1/2 sum V_ksql rho2_ksql. */
+void mcbo_rho(int N, int M, const zc *C, zc *rho1, zc *rho2)
+{
+    long long *tab = (long long *)malloc(sizeof(long long) * (size_t)(N + 1) * (M + 1));
+    mcbo_binom_table(N, M, tab);
+    const long long nc = NC(tab, M, N, M);
+    for (int i = 0; i < M * M; ++i) rho1[i] = 0.0;
+    for (long long i = 0; i < (long long)M * M * M * M; ++i) rho2[i] = 0.0;
+    for (long long g = 0; g < nc; ++g) {
+        int n[MCBO_MAXM];
+        mcbo_unrank(N, M, tab, g, n);
+        const zc cg = conj(C[g]);
+        for (int k = 0; k < M; ++k) {
+            if (n[k] < 1) continue;
+            for (int l = 0; l < M; ++l) {
+                if (l == k) {
+                    rho1[k * M + k] += cg * (double)n[k] * C[g];
+                } else {
+                    double amp = sqrt((double)((long long)n[k] * (n[l] + 1)));
+                    n[k] -= 1; n[l] += 1;
+                    long long b = mcbo_rank(N, M, tab, n);
+                    n[l] -= 1; n[k] += 1;
+                    rho1[k * M + l] += cg * amp * C[b];
+                }
+            }
+        }
+        for (int k = 0; k < M; ++k)
+            for (int s = 0; s < M; ++s) {
+                long long f1 = (long long)n[k] * (n[s] - (k == s ? 1 : 0));
+                if (f1 <= 0) continue;
+                n[k] -= 1; n[s] -= 1;               /* n is now m */
+                for (int q = 0; q < M; ++q)
+                    for (int l = 0; l < M; ++l) {
+                        long long f2 = (long long)(n[q] + 1) * (n[l] + 1 + (q == l ? 1 : 0));
+                        double amp = sqrt((double)(f1 * f2));
+                        n[q] += 1; n[l] += 1;
+                        long long b = mcbo_rank(N, M, tab, n);
+                        n[l] -= 1; n[q] -= 1;
+                        rho2[((k * M + s) * M + q) * M + l] += cg * amp * C[b];
+                    }
+                n[s] += 1; n[k] += 1;
+            }
+    }
+    free(tab);
 }
 
 int mcbo_max_threads(void)
