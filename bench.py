@@ -410,6 +410,23 @@ def run_gpu(args):
             except Exception as ex:  # report, never hide
                 var[name] = {"error": str(ex)}
         line["variants"] = var
+        # density matrices of the same state: one real SYRK (2P x 2P x nc2) on the DMMA path
+        try:
+            for _ in range(3):
+                sp.rho(dCs[0])
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            reps = 10
+            a.record()
+            for i in range(reps):
+                sp.rho(dCs[i % R])
+            b.record(); torch.cuda.synchronize()
+            rho_ms = a.elapsed_time(b) / reps
+            syrk_flop = 2.0 * (2 * tc["P"]) ** 2 * nc2            # full 2P x 2P real product, 2 flop per MAC
+            line["rho"] = {"ms": rho_ms, "configs_per_s": nc / (rho_ms * 1e-3), "launches": int(sp.last_apply_launches()),
+                           "tflops_full_syrk": syrk_flop / (rho_ms * 1e-3) / 1e12,
+                           "gather_GBps": 16.0 * tc["P"] * nc2 / (rho_ms * 1e-3) / 1e9}
+        except Exception as ex:
+            line["rho"] = {"error": str(ex)}
 
     # ---- the oracle beside it (rank 0, N=1 only) ----
     if rank == 0 and world == 1 and not args.no_cpu:

@@ -140,7 +140,19 @@ int  mcb_hc_apply_host(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
                        const mcb_c128* h_C, mcb_c128* h_HC, int mode,
                        mcb_c128* d_C_scratch, mcb_c128* d_HC_scratch, void* d_workspace, void* stream);
 
-/* Number of kernels the last mcb_hc_apply on this space launched (for launch accounting). */
+/* ---- density matrices (Eq. 10-11; index order of App. B) -------------------------
+ *   d_rho1[k*M + l]                 = <Psi| a+_k a_l |Psi>                 (M*M complex, device)
+ *   d_rho2[((k*M+s)*M+q)*M + l]     = <Psi| a+_k a+_s a_q a_l |Psi>        (M^4 complex, device; same index order as V,
+ *                                                                            so <H> = sum T.rho1 + 1/2 sum V.rho2)
+ * for |Psi> = sum_b d_C[b] |n^b> (not normalised by the library).  The two-body matrix is the P x P Gram matrix of
+ * the vectors a_q a_l |Psi> over the (N-2)-particle space, accumulated on the FP64 tensor path without atomics
+ * (deterministic); rho1 follows from sum_s a+_k a+_s a_s a_l = (N-1) a+_k a_l.  Needs FOCK_TABLE if N >= 2 and
+ * mcb_rho_workspace_bytes(sp) bytes of 256-byte aligned device workspace.  M <= MCB_MAX_M_APPLY.  Asynchronous on
+ * `stream`; all pointers 16-byte aligned. */
+long long mcb_rho_workspace_bytes(const mcb_space* sp);
+int  mcb_rho(mcb_space* sp, const mcb_c128* d_C, mcb_c128* d_rho1, mcb_c128* d_rho2, void* d_workspace, void* stream);
+
+/* Number of kernels the last mcb_hc_apply / mcb_rho on this space launched (for launch accounting). */
 int  mcb_last_apply_launches(const mcb_space* sp);
 
 /* ---- measurement support: device time of each kernel of hc_apply --------------------------------------------

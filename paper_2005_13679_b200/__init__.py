@@ -27,6 +27,7 @@ EXPORTS = (
     "mcb_unrank", "mcb_rank", "mcb_structure_bytes", "mcb_build_structure", "mcb_detach_structure",
     "mcb_fock_export", "mcb_map1_export", "mcb_map2_export", "mcb_apply_workspace_bytes",
     "mcb_hc_apply", "mcb_hc_apply_host", "mcb_last_apply_launches", "mcb_timing_enable", "mcb_timing_read", "mcb_fp64_peak", "mcb_strerror", "mcb_last_cuda_error",
+    "mcb_rho_workspace_bytes", "mcb_rho",
 )
 
 _lib = None
@@ -71,6 +72,8 @@ def lib():
         L.mcb_timing_enable.argtypes = [vp, i]
         L.mcb_timing_read.argtypes = [vp, i, vp, vp]
         L.mcb_fp64_peak.argtypes = [i, ctypes.POINTER(ctypes.c_double), vp]
+        L.mcb_rho_workspace_bytes.argtypes = [vp]; L.mcb_rho_workspace_bytes.restype = ll
+        L.mcb_rho.argtypes = [vp, vp, vp, vp, vp, vp]
         L.mcb_strerror.argtypes = [i]; L.mcb_strerror.restype = ctypes.c_char_p
         L.mcb_last_cuda_error.argtypes = []
         _lib = L
@@ -253,6 +256,22 @@ class Space:
                                        mode, self._workspace["dC"].data_ptr(), self._workspace["dHC"].data_ptr(),
                                        self._ws(mode), _stream_ptr(stream)), "mcb_hc_apply_host")
         return out_host
+
+    def rho(self, C, stream=None):
+        """(rho1 [M,M], rho2 [M,M,M,M]) complex128 device tensors: <a+_k a_l>, <a+_k a+_s a_q a_l> of the state C."""
+        torch = _torch()
+        if C.dtype != torch.complex128 or not C.is_cuda or not C.is_contiguous() or C.numel() != self.nc:
+            raise ValueError("C must be a contiguous complex128 CUDA tensor of length nc")
+        need = lib().mcb_rho_workspace_bytes(self._h)
+        if need < 0:
+            raise McbError(int(need), "mcb_rho_workspace_bytes")
+        ws = self._workspace.get("rho")
+        if ws is None or ws.numel() < need:
+            ws = self._workspace["rho"] = torch.empty(int(need), dtype=torch.uint8, device=self.device)
+        r1 = torch.empty((self.M, self.M), dtype=torch.complex128, device=self.device)
+        r2 = torch.empty((self.M,) * 4, dtype=torch.complex128, device=self.device)
+        _check(lib().mcb_rho(self._h, C.data_ptr(), r1.data_ptr(), r2.data_ptr(), ws.data_ptr(), _stream_ptr(stream)), "mcb_rho")
+        return r1, r2
 
     def timing_enable(self, on: bool = True):
         _check(lib().mcb_timing_enable(self._h, 1 if on else 0), "mcb_timing_enable")
