@@ -205,9 +205,10 @@ __global__ void k_rho_expand(const double2* __restrict__ G, const double2* __res
 // =========================================================================================================
 static int rho_grid(const mcb_space* sp)
 {
+    // persistent CTAs per SM the kernel is shaped for (registers / shared memory): 4 for M <= 5, 2 up to M = 8, else 1
     int sms = 0;
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, sp->device) != cudaSuccess || sms < 1) sms = 148;
-    return 2 * sms;
+    return (sp->M <= 5 ? 4 : (sp->M <= 8 ? 2 : 1)) * sms;
 }
 static int rho_rows(int M) { const int P = M * (M + 1) / 2; return (2 * P + 7) / 8 * 8; }
 // partial matrices per CTA: one per warp when K is split (RhoCfg::SPLIT_K: at most 16 block pairs)
