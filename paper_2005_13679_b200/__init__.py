@@ -27,7 +27,7 @@ EXPORTS = (
     "mcb_unrank", "mcb_rank", "mcb_structure_bytes", "mcb_build_structure", "mcb_detach_structure",
     "mcb_fock_export", "mcb_map1_export", "mcb_map2_export", "mcb_apply_workspace_bytes",
     "mcb_hc_apply", "mcb_hc_apply_host", "mcb_last_apply_launches", "mcb_timing_enable", "mcb_timing_read", "mcb_fp64_peak", "mcb_strerror", "mcb_last_cuda_error",
-    "mcb_rho_workspace_bytes", "mcb_rho",
+    "mcb_rho_workspace_bytes", "mcb_rho", "mcb_lanczos_workspace_bytes", "mcb_lanczos",
 )
 
 _lib = None
@@ -74,6 +74,8 @@ def lib():
         L.mcb_fp64_peak.argtypes = [i, ctypes.POINTER(ctypes.c_double), vp]
         L.mcb_rho_workspace_bytes.argtypes = [vp]; L.mcb_rho_workspace_bytes.restype = ll
         L.mcb_rho.argtypes = [vp, vp, vp, vp, vp, vp]
+        L.mcb_lanczos_workspace_bytes.argtypes = [vp, i]; L.mcb_lanczos_workspace_bytes.restype = ll
+        L.mcb_lanczos.argtypes = [vp, vp, vp, vp, i, i, ctypes.c_double, vp, vp, ctypes.POINTER(i), vp, vp, vp]
         L.mcb_strerror.argtypes = [i]; L.mcb_strerror.restype = ctypes.c_char_p
         L.mcb_last_cuda_error.argtypes = []
         _lib = L
@@ -272,6 +274,27 @@ class Space:
         r2 = torch.empty((self.M,) * 4, dtype=torch.complex128, device=self.device)
         _check(lib().mcb_rho(self._h, C.data_ptr(), r1.data_ptr(), r2.data_ptr(), ws.data_ptr(), _stream_ptr(stream)), "mcb_rho")
         return r1, r2
+
+    def lanczos(self, T, V, v0, kmax: int, mode: int = AUTO, breakdown: float = 1e-12, stream=None):
+        """(alpha [k], beta [k]) of the Lanczos tridiagonalisation of H started at the device vector v0 (k <= kmax steps)."""
+        torch = _torch()
+        T = _host_c128(T, (self.M, self.M))
+        V = _host_c128(V, (self.M,) * 4)
+        if v0.dtype != torch.complex128 or not v0.is_cuda or not v0.is_contiguous() or v0.numel() != self.nc:
+            raise ValueError("v0 must be a contiguous complex128 CUDA tensor of length nc")
+        need = lib().mcb_lanczos_workspace_bytes(self._h, kmax)
+        if need < 0:
+            raise McbError(int(need), "mcb_lanczos_workspace_bytes")
+        ws = self._workspace.get("lanczos")
+        if ws is None or ws.numel() < need:
+            ws = self._workspace["lanczos"] = torch.empty(int(need), dtype=torch.uint8, device=self.device)
+        alpha = np.zeros(kmax, dtype=np.float64)
+        beta = np.zeros(kmax, dtype=np.float64)
+        k = ctypes.c_int(0)
+        _check(lib().mcb_lanczos(self._h, T.ctypes.data, V.ctypes.data, v0.data_ptr(), kmax, mode, breakdown,
+                                 alpha.ctypes.data, beta.ctypes.data, ctypes.byref(k), ws.data_ptr(), self._ws(mode),
+                                 _stream_ptr(stream)), "mcb_lanczos")
+        return alpha[:k.value], beta[:k.value]
 
     def timing_enable(self, on: bool = True):
         _check(lib().mcb_timing_enable(self._h, 1 if on else 0), "mcb_timing_enable")
