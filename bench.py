@@ -427,6 +427,18 @@ def run_gpu(args):
                            "gather_GBps": 16.0 * tc["P"] * nc2 / (rho_ms * 1e-3) / 1e9}
         except Exception as ex:
             line["rho"] = {"error": str(ex)}
+        # Lanczos with full re-orthogonalisation (NEXT-2): 16 steps from C, synchronous API
+        try:
+            import time
+            ksteps = 16
+            sp.lanczos(T, V, dCs[0], 4, mode=mode)
+            torch.cuda.synchronize(); t0 = time.perf_counter()
+            al, be = sp.lanczos(T, V, dCs[0], ksteps, mode=mode)
+            torch.cuda.synchronize(); dt = time.perf_counter() - t0
+            line["lanczos"] = {"steps": int(len(al)), "ms_per_step": dt * 1e3 / max(1, len(al)), "alpha0": float(al[0]),
+                               "note": "wall clock of the synchronous call: H.C + two Gram-Schmidt passes over all previous vectors + host read-backs per step"}
+        except Exception as ex:
+            line["lanczos"] = {"error": str(ex)}
 
     # ---- the oracle beside it (rank 0, N=1 only) ----
     if rank == 0 and world == 1 and not args.no_cpu:

@@ -1,0 +1,73 @@
+"""GPU parity of mcb_lanczos against the numpy Lanczos oracle and exact diagonalisation."""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+import workloads
+from oracle import brute
+from oracle import lanczos as olz
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def mcb():
+    import paper_2005_13679_b200 as m
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    m.lib()
+    return m
+
+
+@pytest.mark.parametrize("N,M,kind", [(3, 3, "dense"), (5, 5, "ll"), (6, 4, "dense"), (8, 7, "ll"), (4, 9, "dense"), (1, 4, "dense")])
+def test_lanczos_matches_oracle(mcb, N, M, kind):
+    sp = mcb.Space(N, M)
+    nc = sp.nc
+    T, V, C = workloads.make_small_inputs(N, M, nc, seed=300 + N + M, kind=kind)
+    sp.build_structure(mcb.FOCK_TABLE)
+    k = min(nc, 30)
+    a_ref, b_ref, _ = olz.lanczos(N, M, T, V, C, k)
+    a, b = sp.lanczos(T, V, torch.from_numpy(C).cuda(), k)
+    assert len(a) == len(a_ref)
+    scale = max(1.0, np.abs(a_ref).max())
+    # the recurrence amplifies rounding differences as Ritz values converge: compare the first steps tightly, the
+    # extremal Ritz value (what the method is for) over the whole run
+    e = min(8, len(a))
+    assert np.abs(a[:e] - a_ref[:e]).max() < 1e-9 * scale and np.abs(b[:e] - b_ref[:e]).max() < 1e-9 * scale
+    assert abs(olz.ritz_values(a, b)[0] - olz.ritz_values(a_ref, b_ref)[0]) < 1e-9 * scale
+    if k == nc:                                               # complete Krylov space: the whole spectrum of the dense H
+        H, _ = brute.dense_H(N, M, T, V)
+        assert np.abs(olz.ritz_values(a, b) - np.linalg.eigvalsh(H)).max() < 1e-8 * scale
+    sp.close()
+
+
+def test_lanczos_lieb_liniger_ground_state_vs_ed(mcb):
+    # the paper's end-to-end use, shrunk: N = 5 bosons, M = 5 plane waves, g = 10
+    N, M = 5, 5
+    sp = mcb.Space(N, M)
+    T, V, _ = workloads.lieb_liniger_TV(M)
+    H, _ = brute.dense_H(N, M, T, V)
+    e_ed = np.linalg.eigvalsh(H)[0]
+    sp.build_structure(mcb.FOCK_TABLE)
+    v0 = workloads.random_normalised_C(sp.nc, np.random.default_rng(11))
+    a, b = sp.lanczos(T, V, torch.from_numpy(v0).cuda(), 60)
+    assert abs(olz.ritz_values(a, b)[0] - e_ed) < 1e-9 * abs(e_ed)
+    sp.close()
+
+
+def test_lanczos_full_size_lieb_liniger_runs_and_converges(mcb):
+    # configs[1] (N = 100, M = 5, nc = 4.6e6): 24 steps; the lowest Ritz value can only go down as the space grows
+    c, T, V, (C,) = workloads.make_inputs(1)
+    sp = mcb.Space(c.N, c.M)
+    sp.build_structure(mcb.FOCK_TABLE)
+    a, b = sp.lanczos(T, V, torch.from_numpy(C).cuda(), 24)
+    assert len(a) == 24 and np.isfinite(a).all() and (b > 0).all()
+    lows = [olz.ritz_values(a[:k], b[:k])[0] for k in range(1, 25)]
+    assert all(lows[i + 1] <= lows[i] + 1e-9 * abs(lows[0]) for i in range(23))
+    # alpha_0 is the Rayleigh quotient <C|H|C> of the start vector
+    HC = sp.hc_apply(T, V, torch.from_numpy(C).cuda())
+    assert abs(a[0] - torch.vdot(torch.from_numpy(C).cuda(), HC).real.item()) < 1e-9 * abs(a[0])
+    sp.close()
