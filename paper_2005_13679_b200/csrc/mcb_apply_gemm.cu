@@ -40,7 +40,7 @@ template <int M> struct GemmCfg {
     static constexpr int NRB = cdiv(RB, WR);
     static constexpr int WC = WR >= 4 ? 1 : (WR >= 2 ? 2 : 4);
     static constexpr int NWC = WR * WC;                     // consumer warps
-    static constexpr int NWP = 4;                           // producer warps
+    static constexpr int NWP = (EMBED || M >= 11) ? 4 : 8;  // producer warps (measured: P = 55 wants 8, P = 78 wants 4)
     static constexpr int NPT = NWP * 32;                    // producer threads
     static constexpr int TM = EMBED ? 128 : 64;             // intermediates per tile
     static constexpr int LD = TM + 4;                       // smem row stride (doubles): LD % 16 == 4 -> conflict-free B frags
@@ -51,7 +51,7 @@ template <int M> struct GemmCfg {
     static constexpr int STAGE = NPLANES * DROWS * LD + 2 * M * TM;   // doubles per stage: D planes, R1, R2
     static constexpr int STAGES = 2;
     static constexpr int MINB = (M <= 6) ? 2 : 1;           // CTAs per SM the register budget is shaped for
-    static constexpr int GATHER_BATCH = 8;                  // C gathers in flight per producer thread
+    static constexpr int GATHER_BATCH = (M >= 11) ? 13 : 8; // C gathers in flight per producer thread
     static constexpr int A_ROWS = RB * 8, A_COLS = NK * 4;  // padded coefficient matrix (row-major), x PER matrices
     static constexpr size_t SMEM = (size_t)STAGES * STAGE * sizeof(double) + 2 * STAGES * sizeof(unsigned long long);
     static_assert(NPT % TM == 0 && NPARTS >= 1, "producer mapping");
