@@ -379,7 +379,7 @@ k_hc2_runs(const RunArgs p, const __grid_constant__ RunCoef<M> coef)
                     const int ar = 4 * nb + tig;                         // this lane holds (re, im) of W'[ar][cb * 8 + grp]
                     if (4 * nb + 3 < P || ar < P) {
                         const double f = F[ar * Cfg::FLD + cb * 8 + grp];
-                        W[ar * Cfg::ZLD + cb * 8 + grp] = make_double2(f * acc[cb][nb][0], f * acc[cb][nb][1]);
+                        W[ar * Cfg::ZLD + ((cb * 8 + grp) ^ ((tig >> 1) << 1))] = make_double2(f * acc[cb][nb][0], f * acc[cb][nb][1]);
                     }
                 }
         }
@@ -388,33 +388,39 @@ k_hc2_runs(const RunArgs p, const __grid_constant__ RunCoef<M> coef)
         // ---- phase C: in-run pre-summation (lane = intermediate; slots -1, -2 of lane 0 are the carry slots) and
         //      one store per (class, output) ----
         {
-            const double2* Wl = W + lane;
+            // row a of W' is stored with bit 1 of the slot flipped when bit 1 of a is set: with the 36-slot row stride this
+            // makes the fragment stores of phase B conflict free (rows 4 nb + tig, tig = 0..3, otherwise collide in pairs);
+            // the carry slots -1, -2 (in the padding in front of the row) are not swizzled
+            auto Wat = [&](const int a, const int back) -> const double2& {
+                const int sl = lane - back;
+                return W[a * Cfg::ZLD + (sl >= 0 ? (sl ^ (((a >> 1) & 1) << 1)) : sl)];
+            };
             const int flags = META[Cfg::NCLS * 32 + lane];
             const bool own = flags & 1, last = flags & 2;
             const int mj1 = flags >> 2;
             constexpr int a00 = mcb_pair_index(M, 0, 0), a01 = mcb_pair_index(M, 0, 1), a11 = mcb_pair_index(M, 1, 1);
             if (own) {
                 // class {}: pairs (0,0), (0,1), (1,1)
-                double2 o = Wl[a00 * Cfg::ZLD];
-                if (mj1 >= 1) cadd(o, Wl[a01 * Cfg::ZLD - 1]);
-                if (mj1 >= 2) cadd(o, Wl[a11 * Cfg::ZLD - 2]);
+                double2 o = Wat(a00, 0);
+                if (mj1 >= 1) cadd(o, Wat(a01, 1));
+                if (mj1 >= 2) cadd(o, Wat(a11, 2));
                 double2* dst = p.Hp + META[lane];
                 __stcg(dst, o);
                 if (last) {
-                    double2 e = Wl[a01 * Cfg::ZLD];
-                    if (mj1 >= 1) cadd(e, Wl[a11 * Cfg::ZLD - 1]);
+                    double2 e = Wat(a01, 0);
+                    if (mj1 >= 1) cadd(e, Wat(a11, 1));
                     __stcg(dst + 1, e);
-                    __stcg(dst + 2, Wl[a11 * Cfg::ZLD]);
+                    __stcg(dst + 2, Wat(a11, 0));
                 }
                 // class {h}: pairs (0,h), (1,h)
 #pragma unroll
                 for (int h = 2; h < M; ++h) {
                     const int a0 = mcb_pair_index(M, 0, h), a1 = mcb_pair_index(M, 1, h);
-                    double2 oh = Wl[a0 * Cfg::ZLD];
-                    if (mj1 >= 1) cadd(oh, Wl[a1 * Cfg::ZLD - 1]);
+                    double2 oh = Wat(a0, 0);
+                    if (mj1 >= 1) cadd(oh, Wat(a1, 1));
                     double2* dh = p.Hp + (long long)run_cls_single(h) * p.ldp + META[run_cls_single(h) * 32 + lane];
                     __stcg(dh, oh);
-                    if (last) __stcg(dh + 1, Wl[a1 * Cfg::ZLD]);
+                    if (last) __stcg(dh + 1, Wat(a1, 0));
                 }
                 // class {h,h'}: one pair, one output
 #pragma unroll
@@ -422,16 +428,16 @@ k_hc2_runs(const RunArgs p, const __grid_constant__ RunCoef<M> coef)
 #pragma unroll
                     for (int h2 = h; h2 < M; ++h2) {
                         const int cls = run_cls_pair<M>(h, h2);
-                        __stcg(p.Hp + (long long)cls * p.ldp + META[cls * 32 + lane], Wl[mcb_pair_index(M, h, h2) * Cfg::ZLD]);
+                        __stcg(p.Hp + (long long)cls * p.ldp + META[cls * 32 + lane], Wat(mcb_pair_index(M, h, h2), 0));
                     }
                 }
             }
             if (lane >= 30) {                                            // carry the rows that neighbours read
                 double2* Wn = reinterpret_cast<double2*>(stage_next + Cfg::HEAD_BYTES) + lane - 32;
-                Wn[a01 * Cfg::ZLD] = Wl[a01 * Cfg::ZLD];
-                Wn[a11 * Cfg::ZLD] = Wl[a11 * Cfg::ZLD];
+                Wn[a01 * Cfg::ZLD] = Wat(a01, 0);
+                Wn[a11 * Cfg::ZLD] = Wat(a11, 0);
 #pragma unroll
-                for (int h = 2; h < M; ++h) Wn[mcb_pair_index(M, 1, h) * Cfg::ZLD] = Wl[mcb_pair_index(M, 1, h) * Cfg::ZLD];
+                for (int h = 2; h < M; ++h) Wn[mcb_pair_index(M, 1, h) * Cfg::ZLD] = Wat(mcb_pair_index(M, 1, h), 0);
             }
             __syncwarp();                                                // W' of this stage may now be overwritten
         }
