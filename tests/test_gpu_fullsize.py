@@ -183,3 +183,32 @@ def test_error_paths(mcb):
     assert e.value.status == mcb.EUNSUPPORTED
     sp.close()
     big.close()
+
+
+def test_error_paths_rho_and_lanczos(mcb):
+    sp = mcb.Space(4, 3)
+    C = torch.ones(sp.nc, dtype=torch.complex128, device="cuda")
+    T = np.zeros((3, 3), dtype=np.complex128)
+    V = np.zeros((3,) * 4, dtype=np.complex128)
+    with pytest.raises(mcb.McbError) as e:
+        sp.rho(C)                               # hashing table not built
+    assert e.value.status == mcb.ENOTREADY
+    with pytest.raises(mcb.McbError) as e:
+        sp.lanczos(T, V, C, 4)                  # the apply inside needs the table
+    assert e.value.status == mcb.ENOTREADY
+    sp.build_structure(mcb.FOCK_TABLE)
+    with pytest.raises(mcb.McbError) as e:
+        sp.lanczos(T, V, C, 0)                  # kmax < 1
+    assert e.value.status == mcb.EINVAL
+    with pytest.raises(mcb.McbError) as e:
+        sp.lanczos(T, V, torch.zeros_like(C), 3)        # zero start vector
+    assert e.value.status == mcb.EINVAL
+    a, b = sp.lanczos(T, V, C, 5)               # H = 0: invariant subspace after one step
+    assert len(a) == 1 and a[0] == 0.0 and b[0] == 0.0
+    big = mcb.Space(3, 14)
+    big.build_structure(mcb.FOCK_TABLE)
+    with pytest.raises(mcb.McbError) as e:
+        big.rho(torch.ones(big.nc, dtype=torch.complex128, device="cuda"))
+    assert e.value.status == mcb.EUNSUPPORTED
+    sp.close()
+    big.close()
