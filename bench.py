@@ -234,10 +234,10 @@ class Job:
 # ------------------------------------------------------------------------------------------------------------
 # GPU arm
 # ------------------------------------------------------------------------------------------------------------
-MODES = {"auto": 0, "maps": 1, "rehash": 2, "gemm": 3, "runs": 4}
-MODE_NAMES = {1: "MAPS", 2: "REHASH", 3: "GEMM", 4: "RUNS"}
+MODES = {"auto": 0, "maps": 1, "rehash": 2, "gemm": 3, "runs": 4, "sparse": 5}
+MODE_NAMES = {1: "MAPS", 2: "REHASH", 3: "GEMM", 4: "RUNS", 5: "SPARSE"}
 KERNELS = {1: ["k_hc_direct<M,maps>"], 2: ["k_hc_direct<M,rehash>"], 3: ["k_hc2_contract<M>", "k_hc2_reduce<M>"],
-           4: ["k_hc2_runs<M>"]}
+           4: ["k_hc2_runs<M>"], 5: ["k_hc_sparse<M>"]}
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the committed `ncu --set full`
@@ -303,9 +303,7 @@ def run_gpu(args):
         setup[name + "_bytes"] = sp.structure_bytes(which)
     timed_build(mcb.FOCK_TABLE, "fock_table")
     timed_build(mcb.FOCK_TABLE, "fock_table")            # second build = warm timing
-    mode = MODES[args.mode]
-    if mode == 0:
-        mode = mcb.REHASH if c.N < 2 else (mcb.RUNS if 2 <= c.M <= 5 else mcb.GEMM)     # what MCB_AUTO resolves to
+    mode = sp.resolve_mode(T, V, MODES[args.mode])       # what MCB_AUTO resolves to for these matrix elements
     map_bytes = 0
     if mode == mcb.MAPS:
         timed_build(mcb.MAP1, "map1")
@@ -346,7 +344,14 @@ def run_gpu(args):
     unique_bytes = 32.0 * nc
     fock_bytes = 2.0 * c.M * (nc + nc2)
     alu_peak = fp64_peak_tflops(peaks["sm_max_mhz"])
-    if mode == mcb.MAPS:
+    if mode == mcb.SPARSE:
+        # structured matrix elements: per output one 16-byte gather per non-zero element; the unique bytes are C, HC
+        # and the hashing table of the N-particle space
+        alg_bytes = unique_bytes + 2.0 * c.M * nc
+        roofline = {"bound": "hbm", "kernel": KERNELS[mode][dom], "achieved": alg_bytes / (dom_ms * 1e-3) / 1e9,
+                    "peak": peaks["hbm_gbs"], "unit": "GB/s", "peak_source": peaks["source"], "traffic": None,
+                    "algorithmic_bytes_per_launch": alg_bytes}
+    elif mode == mcb.MAPS:
         alg_bytes = unique_bytes + map_bytes + 2.0 * c.M * nc
         roofline = {"bound": "hbm", "kernel": KERNELS[mode][dom], "achieved": alg_bytes / (dom_ms * 1e-3) / 1e9,
                     "peak": peaks["hbm_gbs"], "unit": "GB/s", "peak_source": peaks["source"], "traffic": None,
@@ -389,7 +394,9 @@ def run_gpu(args):
     # ---- the other variants, short (map-memory vs recompute trade-off) ----
     if args.variants and rank == 0 and world == 1:
         var = {}
-        for name, m in (("REHASH", mcb.REHASH), ("GEMM", mcb.GEMM), ("RUNS", mcb.RUNS), ("MAPS", mcb.MAPS)):
+        for name, m in (("REHASH", mcb.REHASH), ("GEMM", mcb.GEMM), ("RUNS", mcb.RUNS), ("MAPS", mcb.MAPS), ("SPARSE", mcb.SPARSE)):
+            if m == mcb.SPARSE and sp.resolve_mode(T, V) != mcb.SPARSE:
+                continue
             if m == mode or (m in (mcb.GEMM, mcb.RUNS) and c.N < 2) or (m == mcb.RUNS and not 2 <= c.M <= 5):
                 continue
             try:

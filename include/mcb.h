@@ -54,7 +54,9 @@ extern "C" {
 #define MCB_MAP2          2   /* double-jump map, dense [pair(k<=s)][pair(q<=l)][b] layout  */
 
 /* hc_apply modes */
-#define MCB_AUTO          0   /* N < 2: MCB_REHASH; 2 <= M <= MCB_MAX_M_RUNS: MCB_RUNS; else MCB_GEMM              */
+#define MCB_AUTO          0   /* few non-zero elements (at most a quarter of the packed V off its diagonal):
+                                 MCB_SPARSE; else N < 2: MCB_REHASH; 2 <= M <= MCB_MAX_M_RUNS: MCB_RUNS;
+                                 else MCB_GEMM.  The workspace to provide is that of the dense choice.            */
 #define MCB_MAPS          1   /* per-output gather through the stored Map1 + Map2 (the paper's fastest CPU/GPU
                                  variant); needs FOCK_TABLE, MAP1, MAP2                      */
 #define MCB_REHASH        2   /* per-output gather, target indices recomputed on the fly from the hashing table
@@ -68,6 +70,11 @@ extern "C" {
                                  tensor-core contraction), contributions that stay inside a run of the index
                                  order are pre-summed, then a streaming sum over output-indexed planes.
                                  needs FOCK_TABLE and a workspace                                             */
+
+#define MCB_SPARSE        5   /* structured matrix elements (Lieb-Liniger plane waves, Bose-Hubbard):
+                                 per-output gather over the NON-ZERO elements of T and of the packed V only;
+                                 diagonal elements (on-site interaction, T_kk) cost no gather.  At most 1024
+                                 off-diagonal non-zeros (else MCB_EUNSUPPORTED).  needs FOCK_TABLE, no workspace   */
 
 typedef struct mcb_space mcb_space;          /* opaque */
 typedef struct { double re, im; } mcb_c128;
@@ -132,6 +139,11 @@ long long mcb_apply_workspace_bytes(const mcb_space* sp, int mode);
  * Asynchronous on `stream`.  M must be <= MCB_MAX_M_APPLY. */
 int  mcb_hc_apply(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
                   const mcb_c128* d_C, mcb_c128* d_HC, int mode, void* d_workspace, void* stream);
+
+/* The mode mcb_hc_apply(sp, T, V, .., mode, ..) will run: `mode` itself unless it is MCB_AUTO (see MCB_AUTO; depends on
+ * the non-zero pattern of T and V) or the space has N < 2 (MCB_GEMM / MCB_RUNS fall back to MCB_REHASH).  < 0 is an
+ * MCB_E* code. */
+int  mcb_resolve_mode(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, int mode);
 
 /* Same with HOST vectors: copies h_C (nc complex) to d_C_scratch, applies, copies the result from
  * d_HC_scratch to h_HC, and synchronises the stream before returning.  h_C / h_HC should be pinned for

@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libmcb.so")
 
 OK, EINVAL, ERANGE, ENOMEM, ECUDA, ENOTREADY, EUNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
 FOCK_TABLE, MAP1, MAP2 = 0, 1, 2
-AUTO, MAPS, REHASH, GEMM, RUNS = 0, 1, 2, 3, 4
+AUTO, MAPS, REHASH, GEMM, RUNS, SPARSE = 0, 1, 2, 3, 4, 5
 MAX_M, MAX_M_APPLY = 32, 12
 
 EXPORTS = (
@@ -27,7 +27,7 @@ EXPORTS = (
     "mcb_unrank", "mcb_rank", "mcb_structure_bytes", "mcb_build_structure", "mcb_detach_structure",
     "mcb_fock_export", "mcb_map1_export", "mcb_map2_export", "mcb_apply_workspace_bytes",
     "mcb_hc_apply", "mcb_hc_apply_host", "mcb_last_apply_launches", "mcb_timing_enable", "mcb_timing_read", "mcb_fp64_peak", "mcb_strerror", "mcb_last_cuda_error",
-    "mcb_rho_workspace_bytes", "mcb_rho", "mcb_lanczos_workspace_bytes", "mcb_lanczos",
+    "mcb_rho_workspace_bytes", "mcb_rho", "mcb_lanczos_workspace_bytes", "mcb_lanczos", "mcb_resolve_mode",
 )
 
 _lib = None
@@ -72,6 +72,7 @@ def lib():
         L.mcb_timing_enable.argtypes = [vp, i]
         L.mcb_timing_read.argtypes = [vp, i, vp, vp]
         L.mcb_fp64_peak.argtypes = [i, ctypes.POINTER(ctypes.c_double), vp]
+        L.mcb_resolve_mode.argtypes = [vp, vp, vp, i]
         L.mcb_rho_workspace_bytes.argtypes = [vp]; L.mcb_rho_workspace_bytes.restype = ll
         L.mcb_rho.argtypes = [vp, vp, vp, vp, vp, vp]
         L.mcb_lanczos_workspace_bytes.argtypes = [vp, i]; L.mcb_lanczos_workspace_bytes.restype = ll
@@ -225,6 +226,15 @@ class Space:
             w = torch.empty(n, dtype=torch.uint8, device=self.device)
             self._workspace["ws"] = w
         return w.data_ptr()
+
+    def resolve_mode(self, T, V, mode: int = AUTO) -> int:
+        """The mode hc_apply will run for these matrix elements (MCB_AUTO looks at their non-zero pattern)."""
+        T = _host_c128(T, (self.M, self.M))
+        V = _host_c128(V, (self.M,) * 4)
+        r = lib().mcb_resolve_mode(self._h, T.ctypes.data, V.ctypes.data, mode)
+        if r < 0:
+            raise McbError(int(r), "mcb_resolve_mode")
+        return int(r)
 
     def hc_apply(self, T, V, C, out=None, mode: int = AUTO, stream=None):
         """HC = H.C for a complex128 device tensor C [nc]; T [M,M], V [M,M,M,M] host arrays."""

@@ -214,7 +214,8 @@ extern "C" long long mcb_apply_workspace_bytes(const mcb_space* sp, int mode)
 {
     if (!sp) return MCB_EINVAL;
     if (sp->M > MCB_MAX_M_APPLY) return MCB_EUNSUPPORTED;
-    if (mode < MCB_AUTO || mode > MCB_RUNS) return MCB_EINVAL;
+    if (mode < MCB_AUTO || mode > MCB_SPARSE) return MCB_EINVAL;
+    if (mode == MCB_SPARSE) return 0;
     mode = resolve_mode(sp, mode);
     if (mode == MCB_RUNS) return mcb_runs_supported(sp) ? mcb_runs_workspace_bytes(sp) : (long long)MCB_EUNSUPPORTED;
     if (mode != MCB_GEMM) return 0;
@@ -262,7 +263,7 @@ extern "C" int mcb_hc_apply(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
                             const mcb_c128* d_C, mcb_c128* d_HC, int mode, void* d_workspace, void* stream)
 {
     if (!sp || !T || !V || !d_C || !d_HC) return MCB_EINVAL;
-    if (mode < MCB_AUTO || mode > MCB_RUNS) return MCB_EINVAL;
+    if (mode < MCB_AUTO || mode > MCB_SPARSE) return MCB_EINVAL;
     if (sp->M > MCB_MAX_M_APPLY) return MCB_EUNSUPPORTED;
     if ((((uintptr_t)d_C) & 15) || (((uintptr_t)d_HC) & 15)) return MCB_EINVAL;
     {
@@ -271,8 +272,10 @@ extern "C" int mcb_hc_apply(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
         if (c0 < h0 + len && h0 < c0 + len) return MCB_EINVAL;          // overlap
     }
     if (!sp->d_fock) return MCB_ENOTREADY;
-    mode = resolve_mode(sp, mode);
     cudaStream_t st = (cudaStream_t)stream;
+    if (mode == MCB_SPARSE || (mode == MCB_AUTO && mcb_sparse_preferred(sp, T, V)))
+        return mcb_launch_sparse(sp, T, V, d_C, d_HC, st);
+    mode = resolve_mode(sp, mode);
     if (mode == MCB_MAPS && (!sp->d_map1 || (sp->N >= 2 && !sp->d_map2))) return MCB_ENOTREADY;
     if (mode == MCB_RUNS) {
         if (!mcb_runs_supported(sp)) return MCB_EUNSUPPORTED;
@@ -286,6 +289,15 @@ extern "C" int mcb_hc_apply(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
         MCB_DISPATCH_APPLY_M(sp->M, return launch_direct<MT>(sp, use_maps, T, V, d_C, d_HC, st));
     }
     return MCB_EINVAL;
+}
+
+extern "C" int mcb_resolve_mode(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, int mode)
+{
+    if (!sp || !T || !V) return MCB_EINVAL;
+    if (mode < MCB_AUTO || mode > MCB_SPARSE) return MCB_EINVAL;
+    if (sp->M > MCB_MAX_M_APPLY) return MCB_EUNSUPPORTED;
+    if (mode == MCB_SPARSE || (mode == MCB_AUTO && mcb_sparse_preferred(sp, T, V))) return MCB_SPARSE;
+    return resolve_mode(sp, mode);
 }
 
 extern "C" int mcb_hc_apply_host(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,

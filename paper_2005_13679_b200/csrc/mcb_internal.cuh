@@ -81,6 +81,10 @@ long long mcb_runs_workspace_bytes(const mcb_space* sp);
 int mcb_launch_runs(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, const mcb_c128* d_C, mcb_c128* d_HC,
                    void* d_ws, cudaStream_t st);
 
+// MCB_SPARSE mode (mcb_apply_sparse.cu)
+bool mcb_sparse_preferred(mcb_space* sp, const mcb_c128* T, const mcb_c128* V);
+int mcb_launch_sparse(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, const mcb_c128* d_C, mcb_c128* d_HC, cudaStream_t st);
+
 // measurement support (mcb_timing_enable): event i of the current apply's slot, recorded on the apply's stream
 static inline int mcb_tick(mcb_space* sp, int i, cudaStream_t st)
 {

@@ -89,6 +89,21 @@ def lieb_liniger_TV(M: int, g: float = 10.0, L: float = 1.0):
     return np.ascontiguousarray(T), np.ascontiguousarray(V), p
 
 
+def bose_hubbard_TV(M: int, J: float = 1.0, U: float = 4.0, ring: bool = True):
+    """Bose-Hubbard specialisation the paper names: M sites, nearest-neighbour hopping
+    T_kl = -J for |k - l| = 1 (and the ring bond 0 <-> M-1), on-site interaction V_kkkk = U
+    (H = -J sum <kl> a+_k a_l + U/2 sum n_k (n_k - 1)); everything else zero."""
+    T = np.zeros((M, M), dtype=np.complex128)
+    for k in range(M - 1):
+        T[k, k + 1] = T[k + 1, k] = -J
+    if ring and M > 2:
+        T[0, M - 1] = T[M - 1, 0] = -J
+    V = np.zeros((M, M, M, M), dtype=np.complex128)
+    for k in range(M):
+        V[k, k, k, k] = U
+    return T, V
+
+
 def random_normalised_C(nc: int, rng: np.random.Generator) -> np.ndarray:
     """C = randn + i randn, L2-normalised.  complex128 [nc]."""
     C = np.empty(nc, dtype=np.complex128)
@@ -116,6 +131,8 @@ def make_small_inputs(N: int, M: int, nc: int, seed: int, kind: str = "dense", g
     rng = np.random.default_rng(seed)
     if kind == "ll":
         T, V, _ = lieb_liniger_TV(M)
+    elif kind == "bh":
+        T, V = bose_hubbard_TV(M)
     else:
         T = random_hermitian_T(M, rng)
         V = random_general_V(M, rng) if general_V else random_symmetric_V(M, rng)
