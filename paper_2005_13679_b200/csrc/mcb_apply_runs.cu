@@ -64,7 +64,10 @@ template <int M> struct RunCfg {
     static constexpr int WARPS_SM = (int)((227 * 1024 - 2 * 1024) / WARP_BYTES);
     static constexpr int WARPS = WARPS_SM / 2 > 8 ? 8 : WARPS_SM / 2;
     static constexpr int THREADS = (WARPS + 1) * 32;               // + one warp per CTA that only sums
-    static constexpr int SUM_TILE = 512;                           // outputs per sum ticket
+#ifndef RUNS_SUM_TILE
+#define RUNS_SUM_TILE 1024
+#endif
+    static constexpr int SUM_TILE = RUNS_SUM_TILE;                 // outputs per sum ticket
     static constexpr int SUM_U = (NCLS <= 6) ? 4 : 2;                  // outputs in flight per lane
     static constexpr size_t SMEM = WARPS * WARP_BYTES;
     static constexpr int MINB = 2;
@@ -209,6 +212,9 @@ __device__ __forceinline__ void run_sum_tiles(const RunArgs& p, const int lane)
     for (;;) {
         const int t = run_ticket(p.tickets + 1, lane);
         if (t >= p.ntile) break;
+#ifdef RUNS_DEBUG_LAG
+        if (lane == 0) { const int lagk = (int)((((long long)*reinterpret_cast<volatile int*>(p.tickets)) * Cfg::SEG - (long long)t * Cfg::SUM_TILE) >> 10); atomicMax(p.tickets + 3, lagk); }
+#endif
         const int g0 = t * Cfg::SUM_TILE;
         const int g1 = min(g0 + Cfg::SUM_TILE, d.nc);
         const int jmax = (int)__ldg(p.fock.occ + (long long)(M - 1) * p.fock.ld + (g1 - 1));
@@ -241,29 +247,44 @@ __device__ __forceinline__ void run_sum_tiles(const RunArgs& p, const int lane)
             if (lane == 0 && wm > wm_in) atomicMax(p.tickets + 2, wm);
         }
         __threadfence();
+        // rounds of 32 * SUM_U outputs, software-pipelined: the occupations of round r + 1 are loaded before the class-plane
+        // loads of round r are issued, so a round costs one memory latency instead of two
+        int nn[Cfg::SUM_U][M];
+#pragma unroll
+        for (int u = 0; u < Cfg::SUM_U; ++u) {
+            const int g = g0 + u * 32 + lane;
+#pragma unroll
+            for (int j = 0; j < M; ++j) nn[u][j] = g < g1 ? (int)__ldg(p.fock.occ + (long long)j * p.fock.ld + g) : 0;
+        }
 #pragma unroll 1
         for (int gb = g0; gb < g1; gb += 32 * Cfg::SUM_U) {
+            int n[Cfg::SUM_U][M];
+#pragma unroll
+            for (int u = 0; u < Cfg::SUM_U; ++u) {
+                const int gnext = gb + 32 * Cfg::SUM_U + u * 32 + lane;
+#pragma unroll
+                for (int j = 0; j < M; ++j) {
+                    n[u][j] = nn[u][j];
+                    nn[u][j] = gnext < g1 ? (int)__ldg(p.fock.occ + (long long)j * p.fock.ld + gnext) : 0;
+                }
+            }
             // all loads of SUM_U outputs are issued before the first add: SUM_U * NCLS 16-byte loads in flight per lane
             double2 w[Cfg::SUM_U][Cfg::NCLS];
 #pragma unroll
             for (int u = 0; u < Cfg::SUM_U; ++u) {
                 const int g = gb + u * 32 + lane;
-                const bool live = g < g1;
-                int n[M];
-#pragma unroll
-                for (int j = 0; j < M; ++j) n[j] = live ? (int)__ldg(p.fock.occ + (long long)j * p.fock.ld + g) : 0;
-                const int in01 = n[0] + n[1];
+                const int in01 = n[u][0] + n[u][1];
                 const double2* src = p.Hp + g;
                 const double2 zero = make_double2(0.0, 0.0);
                 w[u][0] = (in01 >= 2) ? __ldcg(src) : zero;
 #pragma unroll
                 for (int h = 2; h < M; ++h)
-                    w[u][run_cls_single(h)] = (n[h] >= 1 && in01 >= 1) ? __ldcg(src + (long long)run_cls_single(h) * p.ldp) : zero;
+                    w[u][run_cls_single(h)] = (n[u][h] >= 1 && in01 >= 1) ? __ldcg(src + (long long)run_cls_single(h) * p.ldp) : zero;
 #pragma unroll
                 for (int h = 2; h < M; ++h) {
 #pragma unroll
                     for (int h2 = h; h2 < M; ++h2) {
-                        const bool ok = (h == h2) ? (n[h] >= 2) : (n[h] >= 1 && n[h2] >= 1);
+                        const bool ok = (h == h2) ? (n[u][h] >= 2) : (n[u][h] >= 1 && n[u][h2] >= 1);
                         w[u][run_cls_pair<M>(h, h2)] = ok ? __ldcg(src + (long long)run_cls_pair<M>(h, h2) * p.ldp) : zero;
                     }
                 }
