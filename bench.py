@@ -372,7 +372,8 @@ def run_gpu(args):
     roofline["kernel_share_of_step"] = dom_ms / ms_step
     hbm_unique = {"bytes_per_step": unique_bytes, "achieved_GBps": unique_bytes / (ms_step * 1e-3) / 1e9,
                   "peak_GBps": peaks["hbm_gbs"], "frac": unique_bytes / (ms_step * 1e-3) / 1e9 / peaks["hbm_gbs"],
-                  "note": "unique bytes of C and HC only (32*nc); the step is FP64-ALU bound, see DESIGN.md"}
+                  "note": "unique bytes of C and HC only (32*nc); with dense V the step is bound by FP64 / shared-memory "
+                          "throughput and, in RUNS mode, by the class-plane round trip (roofline.traffic), see DESIGN.md"}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
