@@ -437,6 +437,34 @@ def run_gpu(args):
                            "gather_GBps": 16.0 * tc["P"] * nc2 / (rho_ms * 1e-3) / 1e9}
         except Exception as ex:
             line["rho"] = {"error": str(ex)}
+        # hashing and map-build kernels: HBM-write bound by design; GB/s of the bytes they must move
+        try:
+            def timed(fn, reps=5):
+                fn(); torch.cuda.synchronize()
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record()
+                for _ in range(reps):
+                    fn()
+                b.record(); torch.cuda.synchronize()
+                return a.elapsed_time(b) / reps
+            hk = {}
+            idx_all = torch.arange(nc, dtype=torch.int32, device="cuda")
+            ms = timed(lambda: sp.unrank(idx_all))
+            hk["unrank_all"] = {"ms": ms, "GBps": 4.0 * (c.M + 1) * nc / (ms * 1e-3) / 1e9}
+            occ_all = sp.unrank(idx_all)
+            ms = timed(lambda: sp.rank(occ_all))
+            hk["rank_all"] = {"ms": ms, "GBps": 4.0 * (c.M + 1) * nc / (ms * 1e-3) / 1e9}
+            del occ_all, idx_all
+            ms = timed(lambda: sp.build_structure(mcb.FOCK_TABLE))
+            hk["fock_table"] = {"ms": ms, "GBps": sp.structure_bytes(mcb.FOCK_TABLE) / (ms * 1e-3) / 1e9}
+            free, _ = torch.cuda.mem_get_info()
+            if sp.structure_bytes(mcb.MAP1) < 0.5 * free:
+                ms = timed(lambda: sp.build_structure(mcb.MAP1), reps=3)
+                hk["map1"] = {"ms": ms, "GBps": sp.structure_bytes(mcb.MAP1) / (ms * 1e-3) / 1e9}
+                sp.drop_structure(mcb.MAP1)
+            line["hash_kernels"] = dict(hk, peak_GBps=peaks["hbm_gbs"])
+        except Exception as ex:
+            line["hash_kernels"] = {"error": str(ex)}
         # Lanczos with full re-orthogonalisation (NEXT-2): 16 steps from C, synchronous API
         try:
             import time

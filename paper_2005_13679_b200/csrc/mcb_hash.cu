@@ -91,6 +91,58 @@ __global__ void __launch_bounds__(256) k_fock_table(McbDev d, int Np, int nc_p, 
         if (j < M) { out[(long long)j * ld + b] = (uint16_t)(S[j] - prev); prev = S[j]; }
 }
 
+// Same table for compile-time M: a thread unranks the first of 8 consecutive indices (binary search of the columns
+// of G) and STEPS to the next seven with the successor rule of the order of Eq. (14) (n_1 is the least significant
+// digit, n_0 the remainder): with j* the smallest j >= 1 such that S_{j*-1} >= 1,
+//     n_{j*} += 1,   n_1 .. n_{j*-1} = 0,   n_0 = S_{j*-1} - 1.
+// The 8 occupations of an orbital leave as one 16-byte store: HBM-write bound instead of search bound.
+template <int MT>
+__global__ void __launch_bounds__(256) k_fock_table8(McbDev d, int Np, int nc_p, uint16_t* __restrict__ out, long long ld)
+{
+    static_assert(MT >= 1, "compile-time M");
+    constexpr int M = MT;
+    const int b0 = (blockIdx.x * blockDim.x + threadIdx.x) * 8;
+    if (b0 >= nc_p) return;
+    int n[M];
+    {
+        int S[M];
+        mcb_unrank_prefix<MT>(d.G, d.ldg, M, Np, nc_p, b0, mcb_top_step(Np > 0 ? Np : 1), S);
+        int prev = 0;
+#pragma unroll
+        for (int j = 0; j < M; ++j) { n[j] = S[j] - prev; prev = S[j]; }
+    }
+    unsigned pk[M][4];
+#pragma unroll
+    for (int j = 0; j < M; ++j) { pk[j][0] = pk[j][1] = pk[j][2] = pk[j][3] = 0u; }
+    const int cnt = min(8, nc_p - b0);
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        if (i < cnt) {
+#pragma unroll
+            for (int j = 0; j < M; ++j) pk[j][i >> 1] |= (unsigned)n[j] << (16 * (i & 1));
+        }
+        if (i + 1 < cnt) {                                   // successor
+            int S = n[0], jstar = 0;
+#pragma unroll
+            for (int j = 1; j < M; ++j) { if (jstar == 0 && S >= 1) jstar = j; if (jstar == 0) S += n[j]; }
+#pragma unroll
+            for (int j = 1; j < M; ++j) { if (j < jstar) n[j] = 0; else if (j == jstar) n[j] += 1; }
+            n[0] = S - 1;
+        }
+    }
+    if (cnt == 8) {
+#pragma unroll
+        for (int j = 0; j < M; ++j)
+            *reinterpret_cast<uint4*>(out + (long long)j * ld + b0) = make_uint4(pk[j][0], pk[j][1], pk[j][2], pk[j][3]);
+    } else {
+#pragma unroll
+        for (int j = 0; j < M; ++j)
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+                if (i < cnt) out[(long long)j * ld + b0 + i] = (uint16_t)((pk[j][i >> 1] >> (16 * (i & 1))) & 0xffffu);
+    }
+}
+
 int mcb_launch_unrank(const mcb_space* sp, const int* d_idx, long long batch, int* d_occ, cudaStream_t st)
 {
     const int threads = 256;
@@ -119,8 +171,17 @@ int mcb_launch_fock_table(const mcb_space* sp, int removed, uint16_t* d_out, lon
     const long long n = removed == 0 ? sp->nc : sp->nc2;
     if (Np < 0 || n <= 0) return MCB_OK;
     const int threads = 256;
-    const unsigned blocks = (unsigned)((n + threads - 1) / threads);
-    MCB_DISPATCH_M(sp->M, (k_fock_table<MT><<<blocks, threads, 0, st>>>(sp->dev, Np, (int)n, d_out, ld)));
+    if (sp->M <= 12 && (ld % 8) == 0 && ((uintptr_t)d_out % 16) == 0) {
+        const unsigned blocks = (unsigned)(((n + 7) / 8 + threads - 1) / threads);
+        switch (sp->M) {
+#define MCB_FT8(MM) case MM: k_fock_table8<MM><<<blocks, threads, 0, st>>>(sp->dev, Np, (int)n, d_out, ld); break;
+        MCB_FT8(1) MCB_FT8(2) MCB_FT8(3) MCB_FT8(4) MCB_FT8(5) MCB_FT8(6) MCB_FT8(7) MCB_FT8(8) MCB_FT8(9) MCB_FT8(10) MCB_FT8(11) MCB_FT8(12)
+#undef MCB_FT8
+        }
+    } else {
+        const unsigned blocks = (unsigned)((n + threads - 1) / threads);
+        MCB_DISPATCH_M(sp->M, (k_fock_table<MT><<<blocks, threads, 0, st>>>(sp->dev, Np, (int)n, d_out, ld)));
+    }
     MCB_CHECK_LAUNCH();
     return MCB_OK;
 }
