@@ -19,6 +19,8 @@ torch = pytest.importorskip("torch")
 @pytest.fixture(scope="module")
 def mcb():
     import paper_2005_13679_b200 as m
+    from paper_2005_13679_b200 import build
+    build.build()    # no-op when libmcb.so is current; the library normally travels with the snapshot
     assert torch.cuda.is_available(), "GPU tests need a CUDA device"
     m.lib()
     return m
