@@ -131,7 +131,6 @@ __device__ __forceinline__ void run_prefetch(const RunArgs& p, const int m, cons
                                              unsigned char* __restrict__ stage, const int lane)
 {
     using Cfg = RunCfg<M>;
-    constexpr int P = Cfg::P;
     const McbDev& d = p.d;
     double2* const Z = reinterpret_cast<double2*>(stage + Cfg::HEAD_BYTES) + lane;
     double* const F = reinterpret_cast<double*>(stage + Cfg::HEAD_BYTES + Cfg::Z_BYTES) + lane;

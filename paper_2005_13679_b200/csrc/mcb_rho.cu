@@ -59,7 +59,7 @@ template <int M>
 __global__ void __launch_bounds__(RhoCfg<M>::THREADS) k_rho_gram(const RhoArgs p)
 {
     using Cfg = RhoCfg<M>;
-    constexpr int P = Cfg::P, RB = Cfg::RB, TM = Cfg::TM, LD = Cfg::LD;
+    constexpr int RB = Cfg::RB, TM = Cfg::TM, LD = Cfg::LD;
     extern __shared__ double rho_X[];                                    // [ROWS][LD]
     const McbDev& d = p.d;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
