@@ -55,8 +55,8 @@ extern "C" {
 
 /* hc_apply modes */
 #define MCB_AUTO          0   /* few non-zero elements (at most a quarter of the packed V off its diagonal):
-                                 MCB_SPARSE; else N < 2: MCB_REHASH; 2 <= M <= MCB_MAX_M_RUNS: MCB_RUNS;
-                                 else MCB_GEMM.  The workspace to provide is that of the dense choice.            */
+                                 MCB_SPARSE; else N < 2: MCB_REHASH; 2 <= M <= MCB_MAX_M_RUNS and nc >= 2^20:
+                                 MCB_RUNS; else MCB_GEMM.  The workspace to provide is that of the dense choice.            */
 #define MCB_MAPS          1   /* per-output gather through the stored Map1 + Map2 (the paper's fastest CPU/GPU
                                  variant); needs FOCK_TABLE, MAP1, MAP2                      */
 #define MCB_REHASH        2   /* per-output gather, target indices recomputed on the fly from the hashing table

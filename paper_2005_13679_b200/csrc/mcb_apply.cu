@@ -205,7 +205,10 @@ __global__ void __launch_bounds__(128) k_hc_direct(DirectArgs p)
 
 static int resolve_mode(const mcb_space* sp, int mode)
 {
-    if (mode == MCB_AUTO) return sp->N < 2 ? MCB_REHASH : (mcb_runs_supported(sp) ? MCB_RUNS : MCB_GEMM);
+    // the persistent MCB_RUNS kernel (tickets, flags, a memset) pays off from about a million configurations on
+    // (measured: N = 1000, M = 3, nc = 5.0e5: 52 us against 36 us for MCB_GEMM; N = 2000, nc = 2.0e6: 96 against 128 us)
+    if (mode == MCB_AUTO)
+        return sp->N < 2 ? MCB_REHASH : ((mcb_runs_supported(sp) && sp->nc >= (1LL << 20)) ? MCB_RUNS : MCB_GEMM);
     if ((mode == MCB_GEMM || mode == MCB_RUNS) && sp->N < 2) return MCB_REHASH;   // no (N-2)-particle space: one-body only
     return mode;
 }
