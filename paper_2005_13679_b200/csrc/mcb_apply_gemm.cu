@@ -130,6 +130,16 @@ __global__ void __launch_bounds__(GemmCfg<M>::THREADS, GemmCfg<M>::MINB) k_hc2_c
         const int m_local = ptid % TM;
         const int part = ptid / TM;
         int it = 0;
+        // the occupations of the NEXT tile are loaded while this one is gathered: one memory latency less per tile on the
+        // producers' critical path (consumers were waiting on full stages 22 % of their time, profiles/r1_cfg4_gemm_v2.md)
+        // (not at M >= 11: the 128-register cap of the 448-thread CTA would spill)
+        constexpr bool PREF = M <= 10;
+        int occ_next[M];
+        if (PREF) {
+            const int m0 = blockIdx.x * TM + m_local;
+#pragma unroll
+            for (int j = 0; j < M; ++j) occ_next[j] = (blockIdx.x < p.ntiles && m0 < d.nc2) ? (int)p.fock.occ2[(long long)j * p.fock.ld2 + m0] : 0;
+        }
         for (int tile = blockIdx.x; tile < p.ntiles; tile += gridDim.x, ++it) {
             const int s = it % STAGES;
             double* Dr = smem + s * Cfg::STAGE;                  // [DROWS][LD]   (EMBED: rows 0..P-1 real, P..2P-1 imag)
@@ -145,7 +155,7 @@ __global__ void __launch_bounds__(GemmCfg<M>::THREADS, GemmCfg<M>::MINB) k_hc2_c
                 int run = 0, x = 0, tot1 = 0;
 #pragma unroll
                 for (int j = 0; j < M; ++j) {
-                    const int nj = valid ? (int)p.fock.occ2[(long long)j * p.fock.ld2 + m] : 0;
+                    const int nj = PREF ? occ_next[j] : (valid ? (int)p.fock.occ2[(long long)j * p.fock.ld2 + m] : 0);
                     run += nj;
                     r1[j] = __ldg(d.sq + nj + 1);
                     r2[j] = __ldg(d.sq2 + nj + 2);
@@ -160,6 +170,13 @@ __global__ void __launch_bounds__(GemmCfg<M>::THREADS, GemmCfg<M>::MINB) k_hc2_c
                 int pre = tot1, suf = 0;
 #pragma unroll
                 for (int l = M - 1; l >= 0; --l) { pre -= A1[l]; suf += A2[l]; Y[l] = pre + suf; }
+            }
+            if (PREF) {
+                const int tn = tile + gridDim.x;
+                const int mn = tn * TM + m_local;
+                const bool vn = tn < p.ntiles && mn < d.nc2;
+#pragma unroll
+                for (int j = 0; j < M; ++j) occ_next[j] = vn ? (int)p.fock.occ2[(long long)j * p.fock.ld2 + mn] : 0;
             }
             // gathers are issued in batches of GB per thread; the first batch is in flight BEFORE the wait for the
             // stage, so its latency hides under the consumers draining the previous use of this stage
