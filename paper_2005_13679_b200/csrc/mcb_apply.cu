@@ -91,6 +91,17 @@ __global__ void __launch_bounds__(128) k_hc_direct(DirectArgs p)
     }
     double2 acc = make_double2(0.0, 0.0);
     const double2 cg = p.C[g];
+    // on-the-fly rehashing, few pairs: every prefix sum the index arithmetic can meet is S_j + delta, delta in -2..2, so
+    // the table entries G[j][S_j - 2 .. S_j + 2] are fetched once per output (5 (M-1) look-ups instead of 9 (M-1) per
+    // allowed removal pair); with the pair loops unrolled every use is a compile-time register pick
+    constexpr bool CACHE = !USE_MAPS && P <= 15;
+    int GG[CACHE ? (M > 1 ? M - 1 : 1) : 1][5];
+    if (CACHE) {
+#pragma unroll
+        for (int j = 0; j + 1 < M; ++j)
+#pragma unroll
+            for (int t = 0; t < 5; ++t) GG[j][t] = mcb_ldG(d.G, d.ldg, j, min(max(S[j] + t - 2, 0), d.N));
+    }
 
     // ---- one-body: sum_kl T_kl sqrt(n_k (n_l + 1)) C[g_k^l], diagonal n_k C[g]  (App. B rho_kl, rho_kk) ----
     {
@@ -101,9 +112,9 @@ __global__ void __launch_bounds__(128) k_hc_direct(DirectArgs p)
             for (int j = 0; j < M; ++j) {
                 PM[j] = pm; PP[j] = pp;
                 if (j <= M - 2) {
-                    int g0 = mcb_ldG(d.G, d.ldg, j, S[j]);
-                    int gm = mcb_ldG(d.G, d.ldg, j, S[j] > 0 ? S[j] - 1 : 0);
-                    int gp = mcb_ldG(d.G, d.ldg, j, S[j] < d.N ? S[j] + 1 : d.N);
+                    int g0 = CACHE ? GG[j][2] : mcb_ldG(d.G, d.ldg, j, S[j]);
+                    int gm = CACHE ? GG[j][1] : mcb_ldG(d.G, d.ldg, j, S[j] > 0 ? S[j] - 1 : 0);
+                    int gp = CACHE ? GG[j][3] : mcb_ldG(d.G, d.ldg, j, S[j] < d.N ? S[j] + 1 : d.N);
                     pm += g0 - gm; pp += gp - g0;
                 }
             }
@@ -135,9 +146,14 @@ __global__ void __launch_bounds__(128) k_hc_direct(DirectArgs p)
 
     // ---- two-body: sum over allowed removal pairs (k<=s), then all insertion pairs (q<=l) ----
     if (d.N >= 2) {
-        int a = 0;
+        constexpr int PAIR_UNROLL = CACHE ? M : 1;
+        int a_run = 0;                                                   // pair counter of the rolled loops
+#pragma unroll PAIR_UNROLL
         for (int k = 0; k < M; ++k) {
-            for (int s = k; s < M; ++s, ++a) {
+#pragma unroll PAIR_UNROLL
+            for (int s = CACHE ? 0 : k; s < M; ++s, a_run += CACHE ? 0 : 1) {
+                if (CACHE && s < k) continue;                            // (full trip count so that the loop unrolls)
+                const int a = CACHE ? mcb_pair_index(M, k, s) : a_run;
                 int nk = 0, ns = 0;
 #pragma unroll
                 for (int j = 0; j < M; ++j) { nk = (j == k) ? n[j] : nk; ns = (j == s) ? n[j] : ns; }
@@ -157,9 +173,10 @@ __global__ void __launch_bounds__(128) k_hc_direct(DirectArgs p)
                         X[j] = x;
                         if (!USE_MAPS && j <= M - 2) {
                             const int sp = S[j] - (j >= k) - (j >= s);
-                            const int a0 = mcb_ldG(d.G, d.ldg, j, sp);
-                            A1[j] = mcb_ldG(d.G, d.ldg, j, sp + 1);
-                            A2[j] = mcb_ldG(d.G, d.ldg, j, sp + 2);
+                            const int dlt = 2 - (j >= k) - (j >= s);             // compile time when the pair loops are unrolled
+                            const int a0 = CACHE ? GG[j][dlt] : mcb_ldG(d.G, d.ldg, j, sp);
+                            A1[j] = CACHE ? GG[j][dlt + 1] : mcb_ldG(d.G, d.ldg, j, sp + 1);
+                            A2[j] = CACHE ? GG[j][dlt + 2] : mcb_ldG(d.G, d.ldg, j, sp + 2);
                             x += a0 - A1[j]; tot1 += A1[j];
                         } else { A1[j] = 0; A2[j] = 0; }
                     }
