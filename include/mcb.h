@@ -145,9 +145,12 @@ int  mcb_hc_apply(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
  * MCB_E* code. */
 int  mcb_resolve_mode(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, int mode);
 
-/* Same with HOST vectors: copies h_C (nc complex) to d_C_scratch, applies, copies the result from
- * d_HC_scratch to h_HC, and synchronises the stream before returning.  h_C / h_HC should be pinned for
- * full PCIe bandwidth but need not be. */
+/* Same with HOST vectors: copies h_C (nc complex) to d_C_scratch, applies, brings the result to h_HC, and synchronises
+ * the stream before returning.  h_C / h_HC should be pinned (and must not overlap).  When the mode resolves to MCB_RUNS and
+ * both vectors are pinned the three steps are PIPELINED: C streams in on a stream owned by the space while the kernel,
+ * launched at once on `stream`, waits segment by segment for the prefix of C it needs (an intermediate with top occupation
+ * j gathers only inside the first nc - N_c(N-j-3, M) elements), and the trailing sum writes HC straight into the mapped
+ * host vector; otherwise copy, apply, copy run one after the other through d_HC_scratch. */
 int  mcb_hc_apply_host(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
                        const mcb_c128* h_C, mcb_c128* h_HC, int mode,
                        mcb_c128* d_C_scratch, mcb_c128* d_HC_scratch, void* d_workspace, void* stream);

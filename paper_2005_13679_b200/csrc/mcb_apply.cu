@@ -320,13 +320,50 @@ extern "C" int mcb_resolve_mode(mcb_space* sp, const mcb_c128* T, const mcb_c128
     return resolve_mode(sp, mode);
 }
 
+// Pipelined variant for MCB_RUNS: the contraction walks the intermediates in index order and an intermediate with top
+// occupation j only gathers C inside the first nc - N_c(N-j-3, M) elements, so the kernel is launched at once and waits,
+// segment by segment, for the prefix of C it needs while the host-to-device copy streams in on a second stream; the
+// trailing sum writes HC straight into the (pinned, mapped) host vector.  H2D, compute and D2H overlap.
+// (Measured at configs[2]: 7.3 ms for copy - apply - copy, 4.9 ms pipelined; copying finished pieces of HC back with
+// host-issued DMA behind per-tile flags instead of the zero-copy stores: 5.8 ms.)
+static int hc_apply_host_pipelined(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, const mcb_c128* h_C, mcb_c128* h_HC,
+                                   mcb_c128* d_C_scratch, void* d_workspace, cudaStream_t st, bool* done)
+{
+    *done = false;
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, h_C) != cudaSuccess || at.type != cudaMemoryTypeHost) { cudaGetLastError(); return MCB_OK; }
+    void* d_HC_mapped = nullptr;
+    if (cudaHostGetDevicePointer(&d_HC_mapped, h_HC, 0) != cudaSuccess || !d_HC_mapped) { cudaGetLastError(); return MCB_OK; }
+    if (!sp->copy_stream) {
+        MCB_CUDA(cudaStreamCreateWithFlags(&sp->copy_stream, cudaStreamNonBlocking));
+        MCB_CUDA(cudaEventCreateWithFlags(&sp->ev_a, cudaEventDisableTiming));
+        MCB_CUDA(cudaEventCreateWithFlags(&sp->ev_b, cudaEventDisableTiming));
+        MCB_CUDA(cudaHostAlloc((void**)&sp->h_prog, sizeof(int) * MCB_H2D_CHUNKS, cudaHostAllocDefault));
+    }
+    if (!d_workspace || (((uintptr_t)d_workspace) & 255)) return MCB_EINVAL;
+    int rc = mcb_launch_runs(sp, T, V, d_C_scratch, (mcb_c128*)d_HC_mapped, d_workspace, st, h_C);
+    if (rc != MCB_OK) return rc;
+    MCB_CUDA(cudaEventRecord(sp->ev_b, sp->copy_stream));
+    MCB_CUDA(cudaStreamWaitEvent(st, sp->ev_b, 0));
+    MCB_CUDA(cudaStreamSynchronize(st));
+    *done = true;
+    return MCB_OK;
+}
+
 extern "C" int mcb_hc_apply_host(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
                                  const mcb_c128* h_C, mcb_c128* h_HC, int mode,
                                  mcb_c128* d_C_scratch, mcb_c128* d_HC_scratch, void* d_workspace, void* stream)
 {
-    if (!sp || !h_C || !h_HC || !d_C_scratch || !d_HC_scratch) return MCB_EINVAL;
+    if (!sp || !T || !V || !h_C || !h_HC || !d_C_scratch || !d_HC_scratch) return MCB_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     const size_t len = (size_t)sp->nc * sizeof(mcb_c128);
+    if (sp->d_fock && sp->M <= MCB_MAX_M_APPLY && mode >= MCB_AUTO && mode <= MCB_SPARSE && h_C != h_HC &&
+        mcb_resolve_mode(sp, T, V, mode) == MCB_RUNS && mcb_runs_supported(sp)) {
+        bool done = false;
+        int rc = hc_apply_host_pipelined(sp, T, V, h_C, h_HC, d_C_scratch, d_workspace, st, &done);
+        if (rc != MCB_OK) return rc;
+        if (done) return MCB_OK;                                         // else: vectors not pinned, take the plain path
+    }
     MCB_CUDA(cudaMemcpyAsync(d_C_scratch, h_C, len, cudaMemcpyHostToDevice, st));
     int rc = mcb_hc_apply(sp, T, V, d_C_scratch, d_HC_scratch, mode, d_workspace, stream);
     if (rc != MCB_OK) return rc;

@@ -90,6 +90,7 @@ struct RunArgs {
     int ntile;                 // output tiles of the sum (SUM_TILE outputs each)
     int* flags;                // [nseg] segment s has been contracted and its class planes are visible
     int* tickets;              // [4] next segment, next output tile, verified prefix of flags, pad (zeroed with the flags)
+    const int* c_avail;        // pipelined host apply: number of leading elements of C that have arrived (NULL: all)
 };
 
 __device__ __forceinline__ int run_cls_single(int h) { return 1 + (h - 2); }
@@ -331,6 +332,19 @@ k_hc2_runs(const RunArgs p, const __grid_constant__ RunCoef<M> coef)
             gen_seg = run_ticket(p.tickets, lane);
             gen_ch = 0;
             gen_nch = gen_seg < p.nseg ? (min(gen_seg * Cfg::SEG + Cfg::SEG, d.nc2) - (gen_seg * Cfg::SEG - 2) + 31) >> 5 : 0;
+            if (p.c_avail != nullptr && gen_nch > 0) {
+                // C is still streaming in from the host (mcb_hc_apply_host): an intermediate with top occupation j gathers
+                // targets with n_{M-1} <= j + 2 only, i.e. inside the first nc - N_c(N-j-3, M) elements of C
+                const int last = min(gen_seg * Cfg::SEG + Cfg::SEG, d.nc2) - 1;
+                const int jtop = (int)__ldg(p.fock.occ2 + (long long)(M - 1) * p.fock.ld2 + last);
+                const int need = d.nc - mcb_ldG(d.G, d.ldg, M - 2, max(d.N - (jtop + 2), 0));
+                int have;
+                for (;;) {
+                    asm volatile("ld.acquire.sys.global.s32 %0, [%1];" : "=r"(have) : "l"(p.c_avail) : "memory");
+                    if (have >= need) break;
+                    __nanosleep(2000);
+                }
+            }
             if (gen_nch == 0) { gen_nch = -1; }                          // no work left, stay exhausted
         }
         c.valid = gen_nch > 0;
@@ -494,7 +508,7 @@ long long mcb_runs_workspace_bytes(const mcb_space* sp)
 
 template <int M>
 static int launch_runs(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
-                       const mcb_c128* d_C, mcb_c128* d_HC, void* d_ws, cudaStream_t st)
+                       const mcb_c128* d_C, mcb_c128* d_HC, void* d_ws, cudaStream_t st, const mcb_c128* h_C_src)
 {
     using Cfg = RunCfg<M>;
     constexpr int P = Cfg::P;
@@ -534,6 +548,22 @@ static int launch_runs(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
     }
     { int rc = mcb_tick(sp, 0, st); if (rc) return rc; }
     MCB_CUDA(cudaMemsetAsync(a.tickets, 0, (size_t)(mcb_round_up(a.nseg, 128) + 4) * sizeof(int), st));
+    a.c_avail = nullptr;
+    if (h_C_src) {
+        // pipelined host apply: C streams in on the space's copy stream in MCB_H2D_CHUNKS pieces, each followed by a 4-byte
+        // copy of the number of elements that have arrived; the kernel starts at once and waits per segment (see next_chunk)
+        a.c_avail = a.tickets + 3;
+        MCB_CUDA(cudaEventRecord(sp->ev_a, st));
+        MCB_CUDA(cudaStreamWaitEvent(sp->copy_stream, sp->ev_a, 0));
+        const long long chunk = mcb_round_up((sp->nc + MCB_H2D_CHUNKS - 1) / MCB_H2D_CHUNKS, 4096);
+        int i = 0;
+        for (long long b = 0; b < sp->nc; b += chunk, ++i) {
+            const long long e = b + chunk < sp->nc ? b + chunk : sp->nc;
+            MCB_CUDA(cudaMemcpyAsync((mcb_c128*)d_C + b, h_C_src + b, (size_t)(e - b) * sizeof(mcb_c128), cudaMemcpyHostToDevice, sp->copy_stream));
+            sp->h_prog[i] = (int)e;
+            MCB_CUDA(cudaMemcpyAsync(a.tickets + 3, sp->h_prog + i, sizeof(int), cudaMemcpyHostToDevice, sp->copy_stream));
+        }
+    }
     k_hc2_runs<M><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(a, coef);
     MCB_CHECK_LAUNCH();
     { int rc = mcb_tick(sp, 1, st); if (rc) return rc; }
@@ -543,13 +573,13 @@ static int launch_runs(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
 }
 
 int mcb_launch_runs(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, const mcb_c128* d_C, mcb_c128* d_HC,
-                    void* d_ws, cudaStream_t st)
+                    void* d_ws, cudaStream_t st, const mcb_c128* h_C_src)
 {
     switch (sp->M) {
-    case 2: return launch_runs<2>(sp, T, V, d_C, d_HC, d_ws, st);
-    case 3: return launch_runs<3>(sp, T, V, d_C, d_HC, d_ws, st);
-    case 4: return launch_runs<4>(sp, T, V, d_C, d_HC, d_ws, st);
-    case 5: return launch_runs<5>(sp, T, V, d_C, d_HC, d_ws, st);
+    case 2: return launch_runs<2>(sp, T, V, d_C, d_HC, d_ws, st, h_C_src);
+    case 3: return launch_runs<3>(sp, T, V, d_C, d_HC, d_ws, st, h_C_src);
+    case 4: return launch_runs<4>(sp, T, V, d_C, d_HC, d_ws, st, h_C_src);
+    case 5: return launch_runs<5>(sp, T, V, d_C, d_HC, d_ws, st, h_C_src);
     default: return MCB_EUNSUPPORTED;
     }
 }

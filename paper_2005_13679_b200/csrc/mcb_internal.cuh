@@ -6,6 +6,7 @@
 
 #define MCB_TIMING_RING 512
 #define MCB_MAX_APPLY_KERNELS 3
+#define MCB_H2D_CHUNKS 16
 
 // ---- device-side view of the small per-space constants -------------------------------------------------
 // G[j][s] = binom(s + j, j + 1), j = 0..M-2, s = 0..N: the number of configurations that precede, in the
@@ -44,6 +45,10 @@ struct mcb_space {
     void* d_coef; size_t coef_bytes;
     void* h_coef;              // host scratch for packing
     int last_launches;
+    // pipelined host apply (mcb_hc_apply_host in MCB_RUNS mode): copy stream, fork/join events, pinned progress values
+    cudaStream_t copy_stream;
+    cudaEvent_t ev_a, ev_b;
+    int* h_prog;               // [MCB_H2D_CHUNKS], pinned
     // optional per-kernel timing (mcb_timing_enable): ring of event tuples, one per apply
     int timing;                          // 0 = off
     int t_count;                         // applies recorded since enable (saturates at MCB_TIMING_RING)
@@ -79,7 +84,7 @@ int mcb_launch_gemm(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, const m
 bool mcb_runs_supported(const mcb_space* sp);
 long long mcb_runs_workspace_bytes(const mcb_space* sp);
 int mcb_launch_runs(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, const mcb_c128* d_C, mcb_c128* d_HC,
-                   void* d_ws, cudaStream_t st);
+                   void* d_ws, cudaStream_t st, const mcb_c128* h_C_src = nullptr);
 
 // MCB_SPARSE mode (mcb_apply_sparse.cu)
 bool mcb_sparse_preferred(mcb_space* sp, const mcb_c128* T, const mcb_c128* V);

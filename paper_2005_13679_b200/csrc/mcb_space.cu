@@ -119,6 +119,10 @@ extern "C" void mcb_space_destroy(mcb_space* sp)
     for (int i = 0; i < MCB_TIMING_RING; ++i)
         for (int j = 0; j <= MCB_MAX_APPLY_KERNELS; ++j)
             if (sp->t_ev[i][j]) cudaEventDestroy(sp->t_ev[i][j]);
+    if (sp->copy_stream) cudaStreamDestroy(sp->copy_stream);
+    if (sp->ev_a) cudaEventDestroy(sp->ev_a);
+    if (sp->ev_b) cudaEventDestroy(sp->ev_b);
+    if (sp->h_prog) cudaFreeHost(sp->h_prog);
     if (sp->d_consts) cudaFree(sp->d_consts);
     if (sp->d_coef) cudaFree(sp->d_coef);
     free(sp->h_coef);

@@ -214,3 +214,22 @@ def test_error_paths_rho_and_lanczos(mcb):
     assert e.value.status == mcb.EUNSUPPORTED
     sp.close()
     big.close()
+
+
+def test_apply_host_pipelined_runs_path(mcb):
+    # configs[2] resolves to MCB_RUNS: with pinned vectors mcb_hc_apply_host overlaps H2D, the kernel (which waits per segment
+    # for the prefix of C it needs) and the zero-copy write-back of HC; unpinned vectors take the plain copy-apply-copy path
+    c, T, V, (C,) = workloads.make_inputs(2)
+    sp = mcb.Space(c.N, c.M)
+    sp.build_structure(mcb.FOCK_TABLE)
+    assert sp.resolve_mode(T, V) == mcb.RUNS
+    dev = sp.hc_apply(T, V, torch.from_numpy(C).cuda()).cpu()
+    hC = torch.from_numpy(C).pin_memory()
+    out = torch.empty_like(hC).pin_memory()
+    for _ in range(3):                                   # repeated calls reuse the scratch vectors, streams and flags
+        out.zero_()
+        host = sp.hc_apply_host(T, V, hC, out_host=out)
+        assert torch.equal(dev, host)
+    plain = sp.hc_apply_host(T, V, torch.from_numpy(C))  # pageable memory
+    assert torch.equal(dev, plain)
+    sp.close()
