@@ -20,7 +20,8 @@
  *     enqueued on it and is asynchronous unless stated otherwise.
  *   - the library never allocates or frees caller-visible device memory.  The only device memory it owns
  *     is a few hundred KB of constants per mcb_space (binomial / sqrt tables, packed T,V), allocated in
- *     mcb_space_create and released in mcb_space_destroy.  Hashing table, jump maps and apply workspace
+ *     mcb_space_create and released in mcb_space_destroy (plus, on the first pipelined mcb_hc_apply_host, one copy
+ *     stream, two events and 64 bytes of pinned host memory).  Hashing table, jump maps and apply workspace
  *     live in caller-provided device buffers (e.g. torch tensors) which must stay alive, unmodified,
  *     for as long as the space uses them.
  *   - complex numbers are interleaved (re, im) doubles == C99 double complex == torch.complex128.
