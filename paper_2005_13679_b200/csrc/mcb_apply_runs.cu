@@ -295,7 +295,7 @@ __device__ __forceinline__ void run_sum_tiles(const RunArgs& p, const int lane)
                 double re = 0.0, im = 0.0;
 #pragma unroll
                 for (int k = 0; k < Cfg::NCLS; ++k) { re += w[u][k].x; im += w[u][k].y; }
-                if (g < g1) __stcs(p.HC + g, make_double2(re, im));
+                if (g < g1) __stwt(p.HC + g, make_double2(re, im));
             }
         }
     }
