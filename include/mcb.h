@@ -168,20 +168,31 @@ int  mcb_hc_apply_host(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
 long long mcb_rho_workspace_bytes(const mcb_space* sp);
 int  mcb_rho(mcb_space* sp, const mcb_c128* d_C, mcb_c128* d_rho1, mcb_c128* d_rho2, void* d_workspace, void* stream);
 
-/* ---- Lanczos tridiagonalisation with full re-orthogonalisation (PAPER.md:323-325) -------------------------------
+/* ---- Lanczos tridiagonalisation with full re-orthogonalisation (PAPER.md:323-335) -------------------------------
  * Builds, from the start vector d_v0 (device, nc complex, any non-zero norm), the Krylov basis v_0 .. v_k of H in
  * d_workspace and the real tridiagonal coefficients alpha[0..k-1] (diagonal), beta[0..k-1] (beta[j] = |w_j| couples
  * v_j and v_{j+1}; the last one is the residual norm) on the HOST; the eigenvalues of tridiag(alpha, beta[0..k-2])
- * approximate the extremal eigenvalues of H (the paper solves it with LAPACK on the host).  Every step is one
- * mcb_hc_apply in `mode` plus a twice-applied classical Gram-Schmidt against all previous vectors.  Stops early when
+ * (mcb_tridiag_eigvals) approximate the extremal eigenvalues of H.  Every step is one mcb_hc_apply in `mode` plus a
+ * twice-applied classical Gram-Schmidt against all previous vectors (the paper's full re-orthogonalisation); alpha, beta
+ * and the breakdown test stay on the device, the host looks at them every 8 steps and at the end.  Stops early when
  * beta[j] <= breakdown * max(1, |alpha[0]|) (invariant subspace); *k_done receives the number of steps taken.
- * 1 <= kmax <= 1024.  d_workspace: mcb_lanczos_workspace_bytes(sp, kmax) bytes, 256-byte aligned ((kmax + 2)
- * vectors); d_apply_workspace: as for mcb_hc_apply in `mode`.  SYNCHRONOUS (alpha, beta are read back every step);
- * H must be Hermitian (T, V with the symmetries of BASELINE.json configs) for alpha to be meaningful. */
+ * 0 <= kmax <= 1024; kmax = 0 takes the paper's iteration cap nc / 8 (at most 1024, at least 1) --
+ * mcb_lanczos_steps(sp, kmax) returns the number of steps a given kmax stands for, i.e. the length alpha and beta must have.
+ * d_workspace: mcb_lanczos_workspace_bytes(sp, kmax) bytes, 256-byte aligned ((kmax + 2) vectors + scratch);
+ * d_apply_workspace: as for mcb_hc_apply in `mode`.  SYNCHRONOUS (returns after the last step);
+ * H must be Hermitian (T, V with the symmetries of BASELINE.json configs) for alpha to be meaningful.
+ * MCB_EINVAL also when d_v0 has zero norm. */
+int  mcb_lanczos_steps(const mcb_space* sp, int kmax);
 long long mcb_lanczos_workspace_bytes(const mcb_space* sp, int kmax);
 int  mcb_lanczos(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, const mcb_c128* d_v0, int kmax, int mode,
                  double breakdown, double* alpha, double* beta, int* k_done,
                  void* d_workspace, void* d_apply_workspace, void* stream);
+
+/* Host only: the n eigenvalues, ascending, of the real symmetric tridiagonal matrix with diagonal alpha[0..n-1] and
+ * off-diagonal beta[0..n-2] -- the "tridiagonal system ... solved using LAPACK routines" step of the paper's ground-state
+ * program, here by Sturm-sequence bisection to the last bit (no LAPACK).  eig_out: n doubles.
+ * beta may be NULL when n = 1.  The lowest one, eig_out[0], is the ground-state energy estimate E0. */
+int  mcb_tridiag_eigvals(int n, const double* alpha, const double* beta, double* eig_out);
 
 /* Number of kernels the last mcb_hc_apply / mcb_rho on this space launched (for launch accounting). */
 int  mcb_last_apply_launches(const mcb_space* sp);

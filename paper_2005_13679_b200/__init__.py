@@ -28,6 +28,7 @@ EXPORTS = (
     "mcb_fock_export", "mcb_map1_export", "mcb_map2_export", "mcb_apply_workspace_bytes",
     "mcb_hc_apply", "mcb_hc_apply_host", "mcb_last_apply_launches", "mcb_timing_enable", "mcb_timing_read", "mcb_fp64_peak", "mcb_strerror", "mcb_last_cuda_error",
     "mcb_rho_workspace_bytes", "mcb_rho", "mcb_lanczos_workspace_bytes", "mcb_lanczos", "mcb_resolve_mode",
+    "mcb_lanczos_steps", "mcb_tridiag_eigvals",
 )
 
 _lib = None
@@ -77,6 +78,8 @@ def lib():
         L.mcb_rho.argtypes = [vp, vp, vp, vp, vp, vp]
         L.mcb_lanczos_workspace_bytes.argtypes = [vp, i]; L.mcb_lanczos_workspace_bytes.restype = ll
         L.mcb_lanczos.argtypes = [vp, vp, vp, vp, i, i, ctypes.c_double, vp, vp, ctypes.POINTER(i), vp, vp, vp]
+        L.mcb_lanczos_steps.argtypes = [vp, i]
+        L.mcb_tridiag_eigvals.argtypes = [i, vp, vp, vp]
         L.mcb_strerror.argtypes = [i]; L.mcb_strerror.restype = ctypes.c_char_p
         L.mcb_last_cuda_error.argtypes = []
         _lib = L
@@ -113,6 +116,20 @@ def fp64_peak(kind: int = 0, stream=None) -> float:
     out = ctypes.c_double(0.0)
     _check(lib().mcb_fp64_peak(kind, ctypes.byref(out), _stream_ptr(stream)), "mcb_fp64_peak")
     return float(out.value)
+
+
+def tridiag_eigvals(alpha, beta) -> np.ndarray:
+    """Ascending eigenvalues of the real symmetric tridiagonal matrix with diagonal alpha[0..n-1] and off-diagonal
+    beta[0..n-2] (mcb_tridiag_eigvals: the host-side finish of the Lanczos run).  Host only."""
+    a = np.ascontiguousarray(alpha, dtype=np.float64)
+    n = int(a.size)
+    b = np.ascontiguousarray(np.asarray(beta, dtype=np.float64)[:max(n - 1, 0)])
+    if n > 1 and b.size < n - 1:
+        raise ValueError("beta needs at least n - 1 entries")
+    out = np.empty(n, dtype=np.float64)
+    bb = b if b.size else np.zeros(1)
+    _check(lib().mcb_tridiag_eigvals(n, a.ctypes.data, bb.ctypes.data, out.ctypes.data), "mcb_tridiag_eigvals")
+    return out
 
 
 class Space:
@@ -161,7 +178,8 @@ class Space:
         torch = _torch()
         idx = idx.to(device=self.device, dtype=torch.int32).contiguous()
         occ = torch.empty((idx.numel(), self.M), dtype=torch.int32, device=self.device)
-        _check(lib().mcb_unrank(self._h, idx.data_ptr(), idx.numel(), occ.data_ptr(), _stream_ptr(stream)), "mcb_unrank")
+        with torch.cuda.device(self.device):
+            _check(lib().mcb_unrank(self._h, idx.data_ptr(), idx.numel(), occ.data_ptr(), _stream_ptr(stream)), "mcb_unrank")
         return occ
 
     def rank(self, occ, stream=None):
@@ -169,7 +187,8 @@ class Space:
         torch = _torch()
         occ = occ.to(device=self.device, dtype=torch.int32).contiguous().view(-1, self.M)
         idx = torch.empty((occ.shape[0],), dtype=torch.int32, device=self.device)
-        _check(lib().mcb_rank(self._h, occ.data_ptr(), occ.shape[0], idx.data_ptr(), _stream_ptr(stream)), "mcb_rank")
+        with torch.cuda.device(self.device):
+            _check(lib().mcb_rank(self._h, occ.data_ptr(), occ.shape[0], idx.data_ptr(), _stream_ptr(stream)), "mcb_rank")
         return idx
 
     # -- structures ---------------------------------------------------------------------------------------
@@ -185,7 +204,8 @@ class Space:
         nbytes = self.structure_bytes(which)
         buf = torch.empty(max(nbytes, 256), dtype=torch.uint8, device=self.device)
         assert buf.data_ptr() % 256 == 0
-        _check(lib().mcb_build_structure(self._h, which, buf.data_ptr(), nbytes, _stream_ptr(stream)), "mcb_build_structure")
+        with torch.cuda.device(self.device):
+            _check(lib().mcb_build_structure(self._h, which, buf.data_ptr(), nbytes, _stream_ptr(stream)), "mcb_build_structure")
         self._buffers[which] = buf
         return buf
 
@@ -227,6 +247,13 @@ class Space:
             self._workspace["ws"] = w
         return w.data_ptr()
 
+    def _check_vec(self, t, name: str):
+        """A device vector handed to the library: contiguous complex128, nc elements, on this space's device."""
+        torch = _torch()
+        if (not isinstance(t, torch.Tensor) or t.dtype != torch.complex128 or not t.is_cuda or not t.is_contiguous()
+                or t.numel() != self.nc or t.device != self.device):
+            raise ValueError(f"{name} must be a contiguous complex128 CUDA tensor of length nc = {self.nc} on {self.device}")
+
     def resolve_mode(self, T, V, mode: int = AUTO) -> int:
         """The mode hc_apply will run for these matrix elements (MCB_AUTO looks at their non-zero pattern)."""
         T = _host_c128(T, (self.M, self.M))
@@ -241,12 +268,13 @@ class Space:
         torch = _torch()
         T = _host_c128(T, (self.M, self.M))
         V = _host_c128(V, (self.M,) * 4)
-        if C.dtype != torch.complex128 or not C.is_cuda or not C.is_contiguous() or C.numel() != self.nc:
-            raise ValueError("C must be a contiguous complex128 CUDA tensor of length nc")
+        self._check_vec(C, "C")
         if out is None:
             out = torch.empty_like(C)
-        _check(lib().mcb_hc_apply(self._h, T.ctypes.data, V.ctypes.data, C.data_ptr(), out.data_ptr(), mode,
-                                  self._ws(mode), _stream_ptr(stream)), "mcb_hc_apply")
+        self._check_vec(out, "out")
+        with torch.cuda.device(self.device):
+            _check(lib().mcb_hc_apply(self._h, T.ctypes.data, V.ctypes.data, C.data_ptr(), out.data_ptr(), mode,
+                                      self._ws(mode), _stream_ptr(stream)), "mcb_hc_apply")
         return out
 
     def hc_apply_host(self, T, V, C_host, out_host=None, mode: int = AUTO, stream=None):
@@ -257,23 +285,26 @@ class Space:
         V = _host_c128(V, (self.M,) * 4)
         if isinstance(C_host, np.ndarray):
             C_host = torch.from_numpy(np.ascontiguousarray(C_host, dtype=np.complex128))
-        if C_host.numel() != self.nc or C_host.dtype != torch.complex128 or C_host.is_cuda:
-            raise ValueError("C_host must be a complex128 CPU tensor of length nc")
+        if C_host.numel() != self.nc or C_host.dtype != torch.complex128 or C_host.is_cuda or not C_host.is_contiguous():
+            raise ValueError("C_host must be a contiguous complex128 CPU tensor of length nc")
         if out_host is None:
             out_host = torch.empty_like(C_host)
+        if (not isinstance(out_host, torch.Tensor) or out_host.numel() != self.nc or out_host.dtype != torch.complex128
+                or out_host.is_cuda or not out_host.is_contiguous()):
+            raise ValueError("out_host must be a contiguous complex128 CPU tensor of length nc")
         for name in ("dC", "dHC"):
             if name not in self._workspace:
                 self._workspace[name] = torch.empty(self.nc, dtype=torch.complex128, device=self.device)
-        _check(lib().mcb_hc_apply_host(self._h, T.ctypes.data, V.ctypes.data, C_host.data_ptr(), out_host.data_ptr(),
-                                       mode, self._workspace["dC"].data_ptr(), self._workspace["dHC"].data_ptr(),
-                                       self._ws(mode), _stream_ptr(stream)), "mcb_hc_apply_host")
+        with torch.cuda.device(self.device):
+            _check(lib().mcb_hc_apply_host(self._h, T.ctypes.data, V.ctypes.data, C_host.data_ptr(), out_host.data_ptr(),
+                                           mode, self._workspace["dC"].data_ptr(), self._workspace["dHC"].data_ptr(),
+                                           self._ws(mode), _stream_ptr(stream)), "mcb_hc_apply_host")
         return out_host
 
     def rho(self, C, stream=None):
         """(rho1 [M,M], rho2 [M,M,M,M]) complex128 device tensors: <a+_k a_l>, <a+_k a+_s a_q a_l> of the state C."""
         torch = _torch()
-        if C.dtype != torch.complex128 or not C.is_cuda or not C.is_contiguous() or C.numel() != self.nc:
-            raise ValueError("C must be a contiguous complex128 CUDA tensor of length nc")
+        self._check_vec(C, "C")
         need = lib().mcb_rho_workspace_bytes(self._h)
         if need < 0:
             raise McbError(int(need), "mcb_rho_workspace_bytes")
@@ -282,28 +313,38 @@ class Space:
             ws = self._workspace["rho"] = torch.empty(int(need), dtype=torch.uint8, device=self.device)
         r1 = torch.empty((self.M, self.M), dtype=torch.complex128, device=self.device)
         r2 = torch.empty((self.M,) * 4, dtype=torch.complex128, device=self.device)
-        _check(lib().mcb_rho(self._h, C.data_ptr(), r1.data_ptr(), r2.data_ptr(), ws.data_ptr(), _stream_ptr(stream)), "mcb_rho")
+        with torch.cuda.device(self.device):
+            _check(lib().mcb_rho(self._h, C.data_ptr(), r1.data_ptr(), r2.data_ptr(), ws.data_ptr(), _stream_ptr(stream)), "mcb_rho")
         return r1, r2
 
-    def lanczos(self, T, V, v0, kmax: int, mode: int = AUTO, breakdown: float = 1e-12, stream=None):
-        """(alpha [k], beta [k]) of the Lanczos tridiagonalisation of H started at the device vector v0 (k <= kmax steps)."""
+    def lanczos_steps(self, kmax: int = 0) -> int:
+        """Steps mcb_lanczos takes for `kmax` (0: the paper's cap nc / 8, at most 1024)."""
+        r = int(lib().mcb_lanczos_steps(self._h, kmax))
+        if r < 0:
+            raise McbError(r, "mcb_lanczos_steps")
+        return r
+
+    def lanczos(self, T, V, v0, kmax: int = 0, mode: int = AUTO, breakdown: float = 1e-12, stream=None):
+        """(alpha [k], beta [k]) of the Lanczos tridiagonalisation of H started at the device vector v0 (k <= kmax steps;
+        kmax = 0: the paper's nc / 8).  tridiag_eigvals(alpha, beta[:-1]) gives the Ritz values."""
         torch = _torch()
         T = _host_c128(T, (self.M, self.M))
         V = _host_c128(V, (self.M,) * 4)
-        if v0.dtype != torch.complex128 or not v0.is_cuda or not v0.is_contiguous() or v0.numel() != self.nc:
-            raise ValueError("v0 must be a contiguous complex128 CUDA tensor of length nc")
+        self._check_vec(v0, "v0")
         need = lib().mcb_lanczos_workspace_bytes(self._h, kmax)
         if need < 0:
             raise McbError(int(need), "mcb_lanczos_workspace_bytes")
         ws = self._workspace.get("lanczos")
         if ws is None or ws.numel() < need:
             ws = self._workspace["lanczos"] = torch.empty(int(need), dtype=torch.uint8, device=self.device)
-        alpha = np.zeros(kmax, dtype=np.float64)
-        beta = np.zeros(kmax, dtype=np.float64)
+        steps = self.lanczos_steps(kmax)
+        alpha = np.zeros(steps, dtype=np.float64)
+        beta = np.zeros(steps, dtype=np.float64)
         k = ctypes.c_int(0)
-        _check(lib().mcb_lanczos(self._h, T.ctypes.data, V.ctypes.data, v0.data_ptr(), kmax, mode, breakdown,
-                                 alpha.ctypes.data, beta.ctypes.data, ctypes.byref(k), ws.data_ptr(), self._ws(mode),
-                                 _stream_ptr(stream)), "mcb_lanczos")
+        with torch.cuda.device(self.device):
+            _check(lib().mcb_lanczos(self._h, T.ctypes.data, V.ctypes.data, v0.data_ptr(), kmax, mode, breakdown,
+                                     alpha.ctypes.data, beta.ctypes.data, ctypes.byref(k), ws.data_ptr(), self._ws(mode),
+                                     _stream_ptr(stream)), "mcb_lanczos")
         return alpha[:k.value], beta[:k.value]
 
     def timing_enable(self, on: bool = True):

@@ -338,15 +338,17 @@ static int hc_apply_host_pipelined(mcb_space* sp, const mcb_c128* T, const mcb_c
         MCB_CUDA(cudaStreamCreateWithFlags(&sp->copy_stream, cudaStreamNonBlocking));
         MCB_CUDA(cudaEventCreateWithFlags(&sp->ev_a, cudaEventDisableTiming));
         MCB_CUDA(cudaEventCreateWithFlags(&sp->ev_b, cudaEventDisableTiming));
-        MCB_CUDA(cudaHostAlloc((void**)&sp->h_prog, sizeof(int) * MCB_H2D_CHUNKS, cudaHostAllocDefault));
+        MCB_CUDA(cudaHostAlloc((void**)&sp->h_prog, sizeof(int) * (MCB_H2D_CHUNKS + 4), cudaHostAllocDefault));
     }
     if (!d_workspace || (((uintptr_t)d_workspace) & 255)) return MCB_EINVAL;
+    sp->h_prog[MCB_H2D_CHUNKS] = 0;
     int rc = mcb_launch_runs(sp, T, V, d_C_scratch, (mcb_c128*)d_HC_mapped, d_workspace, st, h_C);
     if (rc != MCB_OK) return rc;
     MCB_CUDA(cudaEventRecord(sp->ev_b, sp->copy_stream));
     MCB_CUDA(cudaStreamWaitEvent(st, sp->ev_b, 0));
     MCB_CUDA(cudaStreamSynchronize(st));
     *done = true;
+    if (sp->h_prog[MCB_H2D_CHUNKS] != 0) return MCB_ECUDA;              // the kernel gave up waiting for a piece of C
     return MCB_OK;
 }
 

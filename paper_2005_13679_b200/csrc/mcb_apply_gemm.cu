@@ -446,14 +446,15 @@ static int launch_gemm(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
     g.W = (double2*)d_ws; g.ldw = gemm_ldw(sp);
     g.ntiles = (int)((sp->nc2 + Cfg::TM - 1) / Cfg::TM);
 
-    static int sm_count = 0, ctas_per_sm = 0;
-    if (!sm_count) {
+    if (!sp->gemm_sms) {                                                 // cached per space (one device, one M)
+        int sm_count = 0, ctas_per_sm = 0;
         MCB_CUDA(cudaFuncSetAttribute(k_hc2_contract<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
         MCB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, k_hc2_contract<M>, Cfg::THREADS, Cfg::SMEM));
         MCB_CUDA(cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, sp->device));
-        if (ctas_per_sm < 1) { sm_count = 0; return MCB_EUNSUPPORTED; }
+        if (ctas_per_sm < 1) return MCB_EUNSUPPORTED;
+        sp->gemm_sms = sm_count; sp->gemm_ctas_per_sm = ctas_per_sm;
     }
-    int grid = sm_count * ctas_per_sm;
+    int grid = sp->gemm_sms * sp->gemm_ctas_per_sm;
     if (grid > g.ntiles) grid = g.ntiles;
     { int rc = mcb_tick(sp, 0, st); if (rc) return rc; }
     k_hc2_contract<M><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(g);

