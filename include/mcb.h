@@ -19,7 +19,8 @@
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  All device work is
  *     enqueued on it and is asynchronous unless stated otherwise.
  *   - the library never allocates or frees caller-visible device memory.  The only device memory it owns
- *     is a few hundred KB of constants per mcb_space (binomial / sqrt tables, packed T,V), allocated in
+ *     is the constants of the mcb_space (binomial / sqrt tables and the staging of the packed T,V: a few hundred KB up to
+ *     12 orbitals, 2 x 16 P^2 bytes beyond -- 18 MB at M = 32), allocated in
  *     mcb_space_create and released in mcb_space_destroy (plus, on the first pipelined mcb_hc_apply_host, one copy
  *     stream, two events and 64 bytes of pinned host memory).  Hashing table, jump maps and apply workspace
  *     live in caller-provided device buffers (e.g. torch tensors) which must stay alive, unmodified,
@@ -42,10 +43,13 @@ extern "C" {
 #define MCB_ENOMEM       -3   /* caller buffer too small / host or device constant allocation failed        */
 #define MCB_ECUDA        -4   /* a CUDA runtime call failed; see mcb_last_cuda_error()                       */
 #define MCB_ENOTREADY    -5   /* a structure the call needs (hashing table, map) has not been built          */
-#define MCB_EUNSUPPORTED -6   /* M > MCB_MAX_M_APPLY for hc_apply, or mode not available for this space       */
+#define MCB_EUNSUPPORTED -6   /* mode not available for this space (see the hc_apply modes)                    */
 
 #define MCB_MAX_M        32   /* hashing and map kernels                                                      */
-#define MCB_MAX_M_APPLY  12   /* hc_apply: packed V (P x P complex, P = M(M+1)/2) must fit on chip            */
+#define MCB_MAX_M_APPLY  32   /* hc_apply, rho, lanczos.  Up to 12 orbitals the packed V (P x P complex, P = M(M+1)/2)
+                                 lives on chip and every mode below exists; for 13 <= M <= 32 (the paper's N = 5,
+                                 M <= 25 sweep) a generic path serves MCB_AUTO / MCB_GEMM and the
+                                 other modes return MCB_EUNSUPPORTED                                           */
 #define MCB_MAX_M_RUNS    5   /* MCB_RUNS: the embedded coefficient matrix must fit in register fragments      */
 
 /* structures that live in caller-provided device memory (mcb_structure_bytes / mcb_build_structure) */
@@ -137,7 +141,7 @@ long long mcb_apply_workspace_bytes(const mcb_space* sp, int mode);
  *      packs exactly that part.  T, V are read before the call returns.
  *   d_C, d_HC: device, nc complex each, 16-byte aligned, must not overlap.
  *   d_workspace: device, mcb_apply_workspace_bytes(sp, mode) bytes, 256-byte aligned (may be NULL if 0).
- * Asynchronous on `stream`.  M must be <= MCB_MAX_M_APPLY. */
+ * Asynchronous on `stream`.  M must be <= MCB_MAX_M_APPLY (modes other than MCB_AUTO / MCB_GEMM: M <= 12). */
 int  mcb_hc_apply(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
                   const mcb_c128* d_C, mcb_c128* d_HC, int mode, void* d_workspace, void* stream);
 

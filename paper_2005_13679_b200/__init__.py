@@ -20,7 +20,7 @@ LIB_PATH = os.path.join(_HERE, "libmcb.so")
 OK, EINVAL, ERANGE, ENOMEM, ECUDA, ENOTREADY, EUNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
 FOCK_TABLE, MAP1, MAP2 = 0, 1, 2
 AUTO, MAPS, REHASH, GEMM, RUNS, SPARSE = 0, 1, 2, 3, 4, 5
-MAX_M, MAX_M_APPLY = 32, 12
+MAX_M, MAX_M_APPLY, MAX_M_TILED = 32, 32, 12
 
 EXPORTS = (
     "mcb_space_create", "mcb_space_destroy", "mcb_nc", "mcb_nc_removed", "mcb_binom_table",

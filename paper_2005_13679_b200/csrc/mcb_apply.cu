@@ -235,6 +235,8 @@ extern "C" long long mcb_apply_workspace_bytes(const mcb_space* sp, int mode)
     if (!sp) return MCB_EINVAL;
     if (sp->M > MCB_MAX_M_APPLY) return MCB_EUNSUPPORTED;
     if (mode < MCB_AUTO || mode > MCB_SPARSE) return MCB_EINVAL;
+    if (sp->M > MCB_MAX_M_TILED)                                         // many orbitals: the generic path (mcb_apply_big.cu)
+        return (mode == MCB_AUTO || mode == MCB_GEMM) ? (sp->N >= 2 ? mcb_big_workspace_bytes(sp) : 0) : (long long)MCB_EUNSUPPORTED;
     if (mode == MCB_SPARSE) return 0;
     mode = resolve_mode(sp, mode);
     if (mode == MCB_RUNS) return mcb_runs_supported(sp) ? mcb_runs_workspace_bytes(sp) : (long long)MCB_EUNSUPPORTED;
@@ -291,8 +293,16 @@ extern "C" int mcb_hc_apply(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
         const size_t len = (size_t)sp->nc * sizeof(mcb_c128);
         if (c0 < h0 + len && h0 < c0 + len) return MCB_EINVAL;          // overlap
     }
-    if (!sp->d_fock) return MCB_ENOTREADY;
     cudaStream_t st = (cudaStream_t)stream;
+    if (sp->M > MCB_MAX_M_TILED) {                                       // many orbitals: the generic path (mcb_apply_big.cu)
+        if (mode != MCB_AUTO && mode != MCB_GEMM) return MCB_EUNSUPPORTED;
+        if (sp->N >= 2) {
+            if (!sp->d_fock) return MCB_ENOTREADY;
+            if (!d_workspace || (((uintptr_t)d_workspace) & 255)) return MCB_EINVAL;
+        }
+        return mcb_launch_big(sp, T, V, d_C, d_HC, d_workspace, st);
+    }
+    if (!sp->d_fock) return MCB_ENOTREADY;
     if (mode == MCB_SPARSE || (mode == MCB_AUTO && mcb_sparse_preferred(sp, T, V)))
         return mcb_launch_sparse(sp, T, V, d_C, d_HC, st);
     mode = resolve_mode(sp, mode);
@@ -316,6 +326,7 @@ extern "C" int mcb_resolve_mode(mcb_space* sp, const mcb_c128* T, const mcb_c128
     if (!sp || !T || !V) return MCB_EINVAL;
     if (mode < MCB_AUTO || mode > MCB_SPARSE) return MCB_EINVAL;
     if (sp->M > MCB_MAX_M_APPLY) return MCB_EUNSUPPORTED;
+    if (sp->M > MCB_MAX_M_TILED) return (mode == MCB_AUTO || mode == MCB_GEMM) ? MCB_GEMM : MCB_EUNSUPPORTED;
     if (mode == MCB_SPARSE || (mode == MCB_AUTO && mcb_sparse_preferred(sp, T, V))) return MCB_SPARSE;
     return resolve_mode(sp, mode);
 }

@@ -1,0 +1,367 @@
+// mcb_apply_big.cu -- hc_apply and the density matrices for MANY orbitals (12 < M <= 32): the paper's second sweep, N = 5
+// particles with M up to 25 orbitals, and its ground-state runs N = 5, M = 11 and 21.
+//
+// The packed coefficient matrix Vp (P x P complex, P = M(M+1)/2 up to 528: 4.5 MB) no longer fits on chip, M is a run-time
+// value, and the (N-2)-particle space is small when N is small (N = 5, M = 21: nc = 53,130 but nc2 = 1,771).  Same
+// factorisation through the (N-2)-particle space as MCB_GEMM (mcb_apply_gemm.cu), written for generality:
+//   k_big_gather   D[c][m] = F(m,c) C[index(m + e_q + e_l)], one thread per intermediate m, all P insertion pairs c = (q<=l)
+//                  (index = nc - 1 - X[q] - Y[l], mcb_device.cuh), materialised in the workspace (P x nc2 complex);
+//   k_big_zgemm    W'[a][m] = F(m,a) sum_c Vp[a][c] D[c][m]: a shared-memory tiled complex GEMM, Vp streamed from L2
+//                  (plain FP64 FMAs: at these shapes the whole product is a fraction of a GFLOP);
+//   k_big_reduce   HC[g] = sum over the allowed removal pairs a of W'[a][index2(n^g - e_k - e_s)] -- every W' element is
+//                  read by exactly one g: no atomics.  T rides inside Vp (sum_s a+_s a_s = N), as in MCB_GEMM.
+//   k_big_gram     G[a][c] = sum_m conj(D[a][m]) D[c][m] (split over m, fixed-order finish): rho2 = G, rho1 from the number
+//                  operator -- mcb_rho for M > 12; mcb_lanczos inherits the apply.
+//   N = 1 (no (N-2)-particle space): HC = T.C, a plain M x M mat-vec (k_big_onebody).
+#include <stdlib.h>
+#include <string.h>
+#include "mcb_device.cuh"
+
+#define BIG_THREADS 128
+#define BIG_BM 32                     // rows (a) per GEMM tile
+#define BIG_BN 64                     // columns (m) per GEMM tile
+#define BIG_BK 16
+#define BIG_SPLIT_MAX 64              // partial Gram matrices
+
+struct BigArgs {
+    McbDev d;
+    McbFockView fock;
+    const double2* C;
+    double2* HC;
+    const double2* Vp;         // [P][P] row-major, T folded in
+    double2* D;                // [P][ld2]
+    double2* W;                // [P][ld2]
+    long long ld2;
+    int P;
+};
+
+// prefix sums -> X[q], Y[l] of the double jump from an intermediate (mcb_maps.cu k_map2 has the derivation); run-time M
+__device__ __forceinline__ void big_xy(const McbDev& d, const int* S, int* X, int* Y)
+{
+    const int M = d.M;
+    int x = 0, tot1 = 0;
+    int A1[MCB_MAX_M], A2[MCB_MAX_M];
+    for (int j = 0; j < M; ++j) {
+        X[j] = x;
+        if (j <= M - 2) {
+            const int a0 = mcb_ldG(d.G, d.ldg, j, S[j]);
+            A1[j] = mcb_ldG(d.G, d.ldg, j, S[j] + 1);
+            A2[j] = mcb_ldG(d.G, d.ldg, j, S[j] + 2);
+            x += a0 - A1[j]; tot1 += A1[j];
+        } else { A1[j] = 0; A2[j] = 0; }
+    }
+    int pre = tot1, suf = 0;
+    for (int l = M - 1; l >= 0; --l) { pre -= A1[l]; suf += A2[l]; Y[l] = pre + suf; }
+}
+
+__global__ void __launch_bounds__(BIG_THREADS) k_big_gather(const BigArgs p)
+{
+    const McbDev& d = p.d;
+    const int m = blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= d.nc2) return;
+    const int M = d.M;
+    int S[MCB_MAX_M], X[MCB_MAX_M], Y[MCB_MAX_M];
+    double r1[MCB_MAX_M], r2[MCB_MAX_M];
+    int run = 0;
+    for (int j = 0; j < M; ++j) {
+        const int nj = (int)p.fock.occ2[(long long)j * p.fock.ld2 + m];
+        run += nj; S[j] = run;
+        r1[j] = __ldg(d.sq + nj + 1);
+        r2[j] = __ldg(d.sq2 + nj + 2);
+    }
+    big_xy(d, S, X, Y);
+    const int base = d.nc - 1;
+    int c = 0;
+    for (int q = 0; q < M; ++q)
+        for (int l = q; l < M; ++l, ++c) {
+            const double2 z = __ldg(p.C + (base - X[q] - Y[l]));
+            const double f = (q == l) ? r2[q] : r1[q] * r1[l];
+            p.D[(long long)c * p.ld2 + m] = make_double2(f * z.x, f * z.y);
+        }
+}
+
+// W'[a][m] = F(m,a) sum_c Vp[a][c] D[c][m].  Tile BM x BN per CTA, 128 threads: thread (ty, tx) = (tid / 16, tid % 16) owns
+// rows a = ty + 8 i (i < 4) and columns m = tx + 16 j (j < 4) of the tile: 16 complex accumulators.
+__global__ void __launch_bounds__(BIG_THREADS) k_big_zgemm(const BigArgs p, const unsigned short* __restrict__ pair_k, const unsigned short* __restrict__ pair_s)
+{
+    __shared__ double2 As[BIG_BK][BIG_BM + 1];
+    __shared__ double2 Bs[BIG_BK][BIG_BN];
+    const McbDev& d = p.d;
+    const int P = p.P;
+    const int a0 = blockIdx.y * BIG_BM, m0 = blockIdx.x * BIG_BN;
+    const int tid = threadIdx.x, ty = tid >> 4, tx = tid & 15;
+    double2 acc[4][4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j] = make_double2(0.0, 0.0);
+    for (int k0 = 0; k0 < P; k0 += BIG_BK) {
+        // A tile: Vp[a0 + r][k0 + kk], read along c (contiguous), stored transposed
+        for (int e = tid; e < BIG_BM * BIG_BK; e += BIG_THREADS) {
+            const int r = e / BIG_BK, kk = e % BIG_BK;
+            const int a = a0 + r, c = k0 + kk;
+            As[kk][r] = (a < P && c < P) ? __ldg(p.Vp + (long long)a * P + c) : make_double2(0.0, 0.0);
+        }
+        for (int e = tid; e < BIG_BK * BIG_BN; e += BIG_THREADS) {
+            const int kk = e / BIG_BN, col = e % BIG_BN;
+            const int c = k0 + kk, m = m0 + col;
+            Bs[kk][col] = (c < P && m < d.nc2) ? p.D[(long long)c * p.ld2 + m] : make_double2(0.0, 0.0);
+        }
+        __syncthreads();
+#pragma unroll
+        for (int kk = 0; kk < BIG_BK; ++kk) {
+            double2 a[4], b[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) a[i] = As[kk][ty + 8 * i];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) b[j] = Bs[kk][tx + 16 * j];
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    acc[i][j].x = fma(a[i].x, b[j].x, acc[i][j].x); acc[i][j].x = fma(-a[i].y, b[j].y, acc[i][j].x);
+                    acc[i][j].y = fma(a[i].x, b[j].y, acc[i][j].y); acc[i][j].y = fma(a[i].y, b[j].x, acc[i][j].y);
+                }
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const int a = a0 + ty + 8 * i;
+        if (a >= P) continue;
+        const int k = pair_k[a], s = pair_s[a];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int m = m0 + tx + 16 * j;
+            if (m >= d.nc2) continue;
+            const int mk = (int)p.fock.occ2[(long long)k * p.fock.ld2 + m];
+            double f;
+            if (k == s) f = __ldg(d.sq2 + mk + 2);
+            else f = __ldg(d.sq + mk + 1) * __ldg(d.sq + (int)p.fock.occ2[(long long)s * p.fock.ld2 + m] + 1);
+            p.W[(long long)a * p.ld2 + m] = make_double2(f * acc[i][j].x, f * acc[i][j].y);
+        }
+    }
+}
+
+// HC[g] = sum over allowed removal pairs (k<=s) of W'[pair(k,s)][index2(n^g - e_k - e_s)]; one thread per output
+__global__ void __launch_bounds__(BIG_THREADS) k_big_reduce(const BigArgs p)
+{
+    const McbDev& d = p.d;
+    const int g = blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= d.nc) return;
+    const int M = d.M;
+    int n[MCB_MAX_M], X[MCB_MAX_M], Y[MCB_MAX_M];
+    {
+        int A1[MCB_MAX_M], A2[MCB_MAX_M];
+        int run = 0, x = 0, tot1 = 0;
+        for (int j = 0; j < M; ++j) {
+            n[j] = p.fock.occ[(long long)j * p.fock.ld + g];
+            run += n[j];
+            X[j] = x;
+            if (j <= M - 2) {
+                // prefix sums of n - e_k - e_s: S_j (j < k), S_j - 1 (k <= j < s), S_j - 2 (j >= s)
+                const int a0 = mcb_ldG(d.G, d.ldg, j, run);
+                A1[j] = mcb_ldG(d.G, d.ldg, j, run >= 1 ? run - 1 : 0);
+                A2[j] = mcb_ldG(d.G, d.ldg, j, run >= 2 ? run - 2 : 0);
+                x += a0 - A1[j]; tot1 += A1[j];
+            } else { A1[j] = 0; A2[j] = 0; }
+        }
+        int pre = tot1, suf = 0;
+        for (int l = M - 1; l >= 0; --l) { pre -= A1[l]; suf += A2[l]; Y[l] = pre + suf; }
+    }
+    double re = 0.0, im = 0.0;
+    for (int k = 0; k < M; ++k) {
+        if (n[k] < 1) continue;
+        for (int s = k; s < M; ++s) {
+            if ((k == s) ? (n[k] < 2) : (n[s] < 1)) continue;
+            const double2 w = p.W[(long long)mcb_pair_index(M, k, s) * p.ld2 + (d.nc2 - 1 - X[k] - Y[s])];
+            re += w.x; im += w.y;
+        }
+    }
+    p.HC[g] = make_double2(re, im);
+}
+
+// N = 1: HC = T.C over the M one-particle configurations (Algorithm 1 gives |e_j> the index j)
+__global__ void k_big_onebody(const double2* __restrict__ Tm, const double2* __restrict__ C, double2* __restrict__ HC, int M)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= M) return;
+    double re = 0.0, im = 0.0;
+    for (int l = 0; l < M; ++l) {
+        const double2 t = Tm[k * M + l], c = C[l];
+        re += t.x * c.x - t.y * c.y; im += t.x * c.y + t.y * c.x;
+    }
+    HC[k] = make_double2(re, im);
+}
+
+// partial[z][a][c] = sum over the m-slice z of conj(D[a][m]) D[c][m]; 32 x 32 tile per CTA, 256 threads, 4 elements each
+__global__ void __launch_bounds__(256) k_big_gram(const double2* __restrict__ D, long long ld2, int P, int nc2, int per_split, double2* __restrict__ partial)
+{
+    __shared__ double2 Ra[32][33], Rc[32][33];
+    const int a0 = blockIdx.y * 32, c0 = blockIdx.x * 32;
+    const int tid = threadIdx.x, ty = tid >> 5, tx = tid & 31;
+    const int mlo = blockIdx.z * per_split, mhi = min(nc2, mlo + per_split);
+    double2 acc[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) acc[i] = make_double2(0.0, 0.0);
+    for (int m0 = mlo; m0 < mhi; m0 += 32) {
+        for (int e = tid; e < 32 * 32; e += 256) {
+            const int r = e >> 5, mm = e & 31;
+            const bool ok = m0 + mm < mhi;
+            Ra[r][mm] = (ok && a0 + r < P) ? D[(long long)(a0 + r) * ld2 + m0 + mm] : make_double2(0.0, 0.0);
+            Rc[r][mm] = (ok && c0 + r < P) ? D[(long long)(c0 + r) * ld2 + m0 + mm] : make_double2(0.0, 0.0);
+        }
+        __syncthreads();
+#pragma unroll 8
+        for (int mm = 0; mm < 32; ++mm) {
+            const double2 c = Rc[tx][mm];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const double2 a = Ra[ty + 8 * i][mm];
+                acc[i].x += a.x * c.x + a.y * c.y;
+                acc[i].y += a.x * c.y - a.y * c.x;
+            }
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const int a = a0 + ty + 8 * i, c = c0 + tx;
+        if (a < P && c < P) partial[((long long)blockIdx.z * P + a) * P + c] = acc[i];
+    }
+}
+
+__global__ void k_big_gram_finish(const double2* __restrict__ partial, int nsplit, int P, double2* __restrict__ G)
+{
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= P * P) return;
+    double re = 0.0, im = 0.0;
+    for (int z = 0; z < nsplit; ++z) { const double2 v = partial[(long long)z * P * P + e]; re += v.x; im += v.y; }
+    G[e] = make_double2(re, im);
+}
+
+// =========================================================================================================
+// host
+// =========================================================================================================
+static long long big_ld2(const mcb_space* sp) { return mcb_round_up(sp->nc2 > 0 ? sp->nc2 : 1, 128); }
+
+long long mcb_big_workspace_bytes(const mcb_space* sp)
+{
+    // D and W', P x ld2 complex each
+    return 2 * (long long)sp->P * big_ld2(sp) * (long long)sizeof(double2);
+}
+
+static int big_pair_tables(mcb_space* sp)
+{
+    if (sp->d_pair_ks) return MCB_OK;
+    const int P = sp->P, M = sp->M;
+    unsigned short* h = (unsigned short*)malloc(sizeof(unsigned short) * 2 * (size_t)P);
+    if (!h) return MCB_ENOMEM;
+    int a = 0;
+    for (int k = 0; k < M; ++k)
+        for (int s = k; s < M; ++s, ++a) { h[a] = (unsigned short)k; h[P + a] = (unsigned short)s; }
+    cudaError_t e = cudaMalloc(&sp->d_pair_ks, sizeof(unsigned short) * 2 * (size_t)P);
+    if (e == cudaSuccess) e = cudaMemcpy(sp->d_pair_ks, h, sizeof(unsigned short) * 2 * (size_t)P, cudaMemcpyHostToDevice);
+    free(h);
+    if (e != cudaSuccess) { if (sp->d_pair_ks) { cudaFree(sp->d_pair_ks); sp->d_pair_ks = NULL; } return mcb_set_cuda_error(e); }
+    return MCB_OK;
+}
+
+static void big_args(const mcb_space* sp, const mcb_c128* d_C, mcb_c128* d_HC, void* d_ws, BigArgs& a)
+{
+    a.d = sp->dev; a.fock = sp->fock;
+    a.C = (const double2*)d_C; a.HC = (double2*)d_HC;
+    a.Vp = (const double2*)sp->d_coef;
+    a.ld2 = big_ld2(sp);
+    a.P = sp->P;
+    a.D = (double2*)d_ws;
+    a.W = a.D + (long long)sp->P * a.ld2;
+}
+
+int mcb_launch_big(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, const mcb_c128* d_C, mcb_c128* d_HC, void* d_ws, cudaStream_t st)
+{
+    const int P = sp->P, M = sp->M;
+    if (sp->N < 2) {
+        // one-body only: HC = T.C (M x M)
+        const size_t bytes = sizeof(mcb_c128) * (size_t)M * M;
+        if (bytes > sp->coef_bytes) return MCB_ENOMEM;
+        memcpy(sp->h_coef, T, bytes);
+        MCB_CUDA(cudaMemcpyAsync(sp->d_coef, sp->h_coef, bytes, cudaMemcpyHostToDevice, st));
+        { int rc = mcb_tick(sp, 0, st); if (rc) return rc; }
+        k_big_onebody<<<(M + 63) / 64, 64, 0, st>>>((const double2*)sp->d_coef, (const double2*)d_C, (double2*)d_HC, M);
+        MCB_CHECK_LAUNCH();
+        { int rc = mcb_tick(sp, 1, st); if (rc) return rc; }
+        mcb_tick_done(sp, 1);
+        sp->last_launches = 1;
+        return MCB_OK;
+    }
+    { int rc = big_pair_tables(sp); if (rc) return rc; }
+    // Vp (T folded in), interleaved complex, staged through the space's host scratch
+    const size_t pp = (size_t)P * P;
+    if (sizeof(double) * 4 * pp > sp->coef_bytes) return MCB_ENOMEM;
+    double* h = (double*)sp->h_coef;
+    double* vr = h + 2 * pp;
+    double* vi = vr + pp;
+    mcb_pack_pairs(sp->N, M, T, V, true, vr, vi);
+    for (size_t i = 0; i < pp; ++i) { h[2 * i] = vr[i]; h[2 * i + 1] = vi[i]; }
+    MCB_CUDA(cudaMemcpyAsync(sp->d_coef, h, sizeof(double) * 2 * pp, cudaMemcpyHostToDevice, st));
+    BigArgs a;
+    big_args(sp, d_C, d_HC, d_ws, a);
+    { int rc = mcb_tick(sp, 0, st); if (rc) return rc; }
+    k_big_gather<<<(unsigned)((sp->nc2 + BIG_THREADS - 1) / BIG_THREADS), BIG_THREADS, 0, st>>>(a);
+    MCB_CHECK_LAUNCH();
+    { int rc = mcb_tick(sp, 1, st); if (rc) return rc; }
+    const dim3 grid((unsigned)((sp->nc2 + BIG_BN - 1) / BIG_BN), (unsigned)((P + BIG_BM - 1) / BIG_BM));
+    k_big_zgemm<<<grid, BIG_THREADS, 0, st>>>(a, sp->d_pair_ks, sp->d_pair_ks + P);
+    MCB_CHECK_LAUNCH();
+    { int rc = mcb_tick(sp, 2, st); if (rc) return rc; }
+    k_big_reduce<<<(unsigned)((sp->nc + BIG_THREADS - 1) / BIG_THREADS), BIG_THREADS, 0, st>>>(a);
+    MCB_CHECK_LAUNCH();
+    { int rc = mcb_tick(sp, 3, st); if (rc) return rc; }
+    mcb_tick_done(sp, 3);
+    sp->last_launches = 3;
+    return MCB_OK;
+}
+
+// ---- density matrices for M > 12 ------------------------------------------------------------------------------------
+static int big_nsplit(const mcb_space* sp)
+{
+    long long s = (sp->nc2 + 4095) / 4096;                              // at least 4096 intermediates per slice
+    if (s < 1) s = 1;
+    if (s > BIG_SPLIT_MAX) s = BIG_SPLIT_MAX;
+    return (int)s;
+}
+
+long long mcb_big_rho_workspace_bytes(const mcb_space* sp)
+{
+    const long long pp = (long long)sp->P * sp->P * (long long)sizeof(double2);
+    return (long long)sp->P * big_ld2(sp) * (long long)sizeof(double2)   // D
+           + mcb_round_up((long long)big_nsplit(sp) * pp, 256)          // partial Gram matrices
+           + mcb_round_up(pp, 256);                                     // G
+}
+
+int mcb_launch_rho_big(mcb_space* sp, const mcb_c128* d_C, mcb_c128* d_rho1, mcb_c128* d_rho2, void* d_ws, cudaStream_t st)
+{
+    const int P = sp->P, M = sp->M;
+    const long long pp = (long long)P * P * (long long)sizeof(double2);
+    BigArgs a;
+    big_args(sp, d_C, NULL, d_ws, a);
+    double2* partial = a.D + (long long)P * a.ld2;
+    const int nsplit = big_nsplit(sp);
+    double2* G = (double2*)((char*)partial + mcb_round_up((long long)nsplit * pp, 256));
+    int launches = 0;
+    if (sp->N >= 2) {
+        k_big_gather<<<(unsigned)((sp->nc2 + BIG_THREADS - 1) / BIG_THREADS), BIG_THREADS, 0, st>>>(a);
+        MCB_CHECK_LAUNCH();
+        const int per_split = (int)mcb_round_up((sp->nc2 + nsplit - 1) / nsplit, 32);
+        const dim3 grid((unsigned)((P + 31) / 32), (unsigned)((P + 31) / 32), (unsigned)nsplit);
+        k_big_gram<<<grid, 256, 0, st>>>(a.D, a.ld2, P, (int)sp->nc2, per_split, partial);
+        MCB_CHECK_LAUNCH();
+        k_big_gram_finish<<<(P * P + 255) / 256, 256, 0, st>>>(partial, nsplit, P, G);
+        MCB_CHECK_LAUNCH();
+        launches = 3;
+    }
+    { int rc = mcb_rho_expand_launch(G, d_C, sp->N, M, d_rho1, d_rho2, st); if (rc) return rc; }
+    sp->last_launches = launches + 1;
+    return MCB_OK;
+}

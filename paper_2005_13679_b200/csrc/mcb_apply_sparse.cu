@@ -192,7 +192,7 @@ static int sparse_pack(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, int*
 bool mcb_sparse_preferred(mcb_space* sp, const mcb_c128* T, const mcb_c128* V)
 {
     int n1, n2; size_t bytes;
-    if (sp->M > MCB_MAX_M_APPLY) return false;
+    if (sp->M > MCB_MAX_M_TILED) return false;
     if (sparse_pack(sp, T, V, &n1, &n2, &bytes, true) < 0) return false;
     return 4 * (long long)n2 <= (long long)sp->P * sp->P;             // the M (M - 1) one-body entries never dominate
 }

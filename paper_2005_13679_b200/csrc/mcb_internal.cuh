@@ -7,6 +7,7 @@
 #define MCB_TIMING_RING 512
 #define MCB_MAX_APPLY_KERNELS 3
 #define MCB_H2D_CHUNKS 16
+#define MCB_MAX_M_TILED 12     // up to here the packed coefficient matrix lives on chip (templated kernels); beyond: mcb_apply_big.cu
 
 // ---- device-side view of the small per-space constants -------------------------------------------------
 // G[j][s] = binom(s + j, j + 1), j = 0..M-2, s = 0..N: the number of configurations that precede, in the
@@ -49,6 +50,7 @@ struct mcb_space {
     void* runs_coef;           // host scratch of MCB_RUNS: coefficient matrix + packed Vp (lazily allocated)
     int runs_grid;             // persistent grid of k_hc2_runs on this space's device (0: not yet queried)
     int gemm_sms, gemm_ctas_per_sm;      // same for k_hc2_contract
+    unsigned short* d_pair_ks; // [2][P] pair index -> (k, s), device (M > MCB_MAX_M_TILED only)
     unsigned attr_set;         // bit i: cudaFuncSetAttribute done for kernel family i on this space's device
     // pipelined host apply (mcb_hc_apply_host in MCB_RUNS mode): copy stream, fork/join events, pinned progress values
     cudaStream_t copy_stream;
@@ -90,6 +92,13 @@ bool mcb_runs_supported(const mcb_space* sp);
 long long mcb_runs_workspace_bytes(const mcb_space* sp);
 int mcb_launch_runs(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, const mcb_c128* d_C, mcb_c128* d_HC,
                    void* d_ws, cudaStream_t st, const mcb_c128* h_C_src = nullptr);
+
+// many orbitals, MCB_MAX_M_TILED < M <= MCB_MAX_M_APPLY (mcb_apply_big.cu)
+long long mcb_big_workspace_bytes(const mcb_space* sp);
+int mcb_launch_big(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, const mcb_c128* d_C, mcb_c128* d_HC, void* d_ws, cudaStream_t st);
+long long mcb_big_rho_workspace_bytes(const mcb_space* sp);
+int mcb_launch_rho_big(mcb_space* sp, const mcb_c128* d_C, mcb_c128* d_rho1, mcb_c128* d_rho2, void* d_ws, cudaStream_t st);
+int mcb_rho_expand_launch(const void* d_G, const mcb_c128* d_C, int N, int M, mcb_c128* d_rho1, mcb_c128* d_rho2, cudaStream_t st);
 
 // MCB_SPARSE mode (mcb_apply_sparse.cu)
 bool mcb_sparse_preferred(mcb_space* sp, const mcb_c128* T, const mcb_c128* V);

@@ -214,10 +214,19 @@ static int rho_rows(int M) { const int P = M * (M + 1) / 2; return (2 * P + 7) /
 // partial matrices per CTA: one per warp when K is split (RhoCfg::SPLIT_K: at most 16 block pairs)
 static int rho_parts(int M) { const int rb = rho_rows(M) / 8; return rb * (rb + 1) / 2 <= 16 ? 8 : 1; }
 
+int mcb_rho_expand_launch(const void* d_G, const mcb_c128* d_C, int N, int M, mcb_c128* d_rho1, mcb_c128* d_rho2, cudaStream_t st)
+{
+    const int M4 = M * M * M * M;
+    k_rho_expand<<<(M4 + 127) / 128, 128, 0, st>>>((const double2*)d_G, (const double2*)d_C, N, M, (double2*)d_rho1, (double2*)d_rho2);
+    MCB_CHECK_LAUNCH();
+    return MCB_OK;
+}
+
 extern "C" long long mcb_rho_workspace_bytes(const mcb_space* sp)
 {
     if (!sp) return MCB_EINVAL;
     if (sp->M > MCB_MAX_M_APPLY) return MCB_EUNSUPPORTED;
+    if (sp->M > MCB_MAX_M_TILED) return mcb_big_rho_workspace_bytes(sp);
     const long long rows = rho_rows(sp->M);
     const long long partial = mcb_round_up((long long)rho_grid(sp) * rho_parts(sp->M) * rows * rows * (long long)sizeof(double), 256);
     return partial + mcb_round_up((long long)sp->P * sp->P * (long long)sizeof(double2), 256);
@@ -263,6 +272,7 @@ extern "C" int mcb_rho(mcb_space* sp, const mcb_c128* d_C, mcb_c128* d_rho1, mcb
         return MCB_EINVAL;
     if (sp->N >= 2 && !sp->d_fock) return MCB_ENOTREADY;
     cudaStream_t st = (cudaStream_t)stream;
+    if (sp->M > MCB_MAX_M_TILED) return mcb_launch_rho_big(sp, d_C, d_rho1, d_rho2, d_workspace, st);
     switch (sp->M) {
     case 1: return launch_rho<1>(sp, d_C, d_rho1, d_rho2, d_workspace, st);
     case 2: return launch_rho<2>(sp, d_C, d_rho1, d_rho2, d_workspace, st);

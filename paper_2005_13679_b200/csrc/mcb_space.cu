@@ -26,7 +26,7 @@ extern "C" const char* mcb_strerror(int status)
     case MCB_ENOMEM:       return "buffer too small or allocation failed";
     case MCB_ECUDA:        return "CUDA runtime error (see mcb_last_cuda_error)";
     case MCB_ENOTREADY:    return "required structure (hashing table / jump map) not built";
-    case MCB_EUNSUPPORTED: return "unsupported for this space (M > MCB_MAX_M_APPLY or mode unavailable)";
+    case MCB_EUNSUPPORTED: return "unsupported for this space (mode unavailable for this M or N)";
     default:               return "unknown status";
     }
 }
@@ -125,6 +125,7 @@ extern "C" void mcb_space_destroy(mcb_space* sp)
     if (sp->h_prog) cudaFreeHost(sp->h_prog);
     if (sp->d_consts) cudaFree(sp->d_consts);
     if (sp->d_coef) cudaFree(sp->d_coef);
+    if (sp->d_pair_ks) cudaFree(sp->d_pair_ks);
     free(sp->h_coef);
     free(sp->runs_coef);
     free(sp->h_binom);

@@ -180,9 +180,11 @@ def test_error_paths(mcb):
     big = mcb.Space(3, 14)
     big.build_structure(mcb.FOCK_TABLE)
     Cb = torch.zeros(big.nc, dtype=torch.complex128, device="cuda")
-    with pytest.raises(mcb.McbError) as e:
-        big.hc_apply(np.zeros((14, 14), dtype=np.complex128), np.zeros((14,) * 4, dtype=np.complex128), Cb)
+    with pytest.raises(mcb.McbError) as e:          # 12 < M <= 32: the generic path has no per-output (REHASH) variant
+        big.hc_apply(np.zeros((14, 14), dtype=np.complex128), np.zeros((14,) * 4, dtype=np.complex128), Cb, mode=mcb.REHASH)
     assert e.value.status == mcb.EUNSUPPORTED
+    out = big.hc_apply(np.zeros((14, 14), dtype=np.complex128), np.zeros((14,) * 4, dtype=np.complex128), Cb)
+    assert float(out.abs().max()) == 0.0
     sp.close()
     big.close()
 
@@ -208,11 +210,15 @@ def test_error_paths_rho_and_lanczos(mcb):
     assert e.value.status == mcb.EINVAL
     a, b = sp.lanczos(T, V, C, 5)               # H = 0: invariant subspace after one step
     assert len(a) == 1 and a[0] == 0.0 and b[0] == 0.0
-    big = mcb.Space(3, 14)
+    big = mcb.Space(3, 14)                      # many orbitals: the generic path serves AUTO / GEMM only
     big.build_structure(mcb.FOCK_TABLE)
-    with pytest.raises(mcb.McbError) as e:
-        big.rho(torch.ones(big.nc, dtype=torch.complex128, device="cuda"))
-    assert e.value.status == mcb.EUNSUPPORTED
+    Tb, Vb = np.zeros((14, 14), dtype=np.complex128), np.zeros((14,) * 4, dtype=np.complex128)
+    Cb = torch.ones(big.nc, dtype=torch.complex128, device="cuda")
+    for mode in (mcb.REHASH, mcb.MAPS, mcb.RUNS, mcb.SPARSE):
+        with pytest.raises(mcb.McbError) as e:
+            big.hc_apply(Tb, Vb, Cb, mode=mode)
+        assert e.value.status == mcb.EUNSUPPORTED
+    assert big.resolve_mode(Tb, Vb) == mcb.GEMM
     sp.close()
     big.close()
 
