@@ -131,11 +131,22 @@ def test_hc_apply_runs_many_segments(mcb, N, M):
     sp.build_structure(mcb.FOCK_TABLE)
     dC = torch.from_numpy(C).cuda()
     got = sp.hc_apply(T, V, dC, mode=mcb.RUNS)
-    err = np.abs(got.cpu().numpy() - ref).max()
     # The north-star bound 1e-12 * ||T,V||max * ||C||_1 does not grow with the amplitudes (up to N^2): at N = 2000 it is
-    # 5 ulp of the largest |HC| (~1e5), tighter than ANY reordering of an fp64 sum of 2 P^2 terms can promise.  Beyond
-    # the paper's range (N <= 1000) the bound is the arithmetic one of DESIGN.md section 2: 64 ulp of max|HC|.
-    t = max(tol(T, V, C), 64 * 2.0 ** -53 * np.abs(ref).max()) if N > 1000 else tol(T, V, C)
+    # 5 ulp of the largest |HC| (~1e5).  There the fp64 ORACLE's own rounding, measured against the extended-precision
+    # evaluation of the same definition (oracle/extended.py, pinned in tests/test_oracle_apply.py), is as large as the bound
+    # itself -- no fp64 evaluation can promise it.  So beyond the paper's range (N <= 1000) every mode is
+    # compared with the EXTENDED-precision reference under the arithmetic bound of DESIGN.md section 2, 64 ulp of max|HC|,
+    # and the oracle is held to the same.
+    t = tol(T, V, C)
+    if N > 1000:
+        assert M == 2
+        from oracle import extended
+        truth = extended.hc_apply_m2_longdouble(N, T, V, C)
+        t = 64 * 2.0 ** -53 * float(np.abs(truth).max())
+        assert float(np.abs(ref - truth).max()) > 0.5 * tol(T, V, C)        # the oracle itself is at the north-star bound
+        assert float(np.abs(ref - truth).max()) <= t
+        ref = truth
+    err = float(np.abs(got.cpu().numpy() - ref).max())
     assert err <= t, (err, t)
     assert sp.last_apply_launches() == 1
     # the workspace (class planes, tickets, flags) is reused: a second apply, on a side stream, gives the same bits

@@ -312,3 +312,28 @@ def test_LL_momentum_sector_is_invariant():
     C = np.where(Ptot == 1, C, 0)
     HC, _ = oracle.hc_apply(N, M, T, V, C)
     assert np.abs(HC[Ptot != 1]).max() == 0.0 and np.abs(HC[Ptot == 1]).max() > 0
+
+
+def test_extended_precision_reference_two_orbitals():
+    """oracle.extended (M = 2, numpy longdouble) against the fp64 oracle: the same operator, and the size of the fp64
+    oracle's OWN rounding.  For M = 2 the order of Eq. (14) gives |n_0, n_1> the index n_1 (checked against Algorithm 1).
+    At N = 2000 (beyond the paper's range) the oracle's fp64 error is as large as the north-star tolerance
+    1e-12 * ||T,V||max * ||C||_1 itself: that bound does not grow with the amplitudes (~N^2) and cannot be promised by ANY
+    fp64 evaluation there -- which is why the one GPU test at N = 2000 uses the arithmetic bound."""
+    from oracle import extended
+    assert np.finfo(np.longdouble).nmant >= 63, "needs the x87 extended format"
+    for N in (1, 2, 3, 7, 40, 300):
+        assert (oracle.rank(N, 2, np.stack([N - np.arange(N + 1), np.arange(N + 1)], 1)) == np.arange(N + 1)).all()
+        T, V, C = workloads.make_small_inputs(N, 2, N + 1, seed=4242 + 31 * N + 2, general_V=(N + 2) % 2 == 1)
+        ref, _ = oracle.hc_apply(N, 2, T, V, C)
+        ld = extended.hc_apply_m2_longdouble(N, T, V, C)
+        assert float(np.abs(ref - ld).max()) <= 8 * 2.0 ** -53 * max(1.0, float(np.abs(ref).max())), N
+        assert float(np.abs(ref - ld).max()) <= 0.25 * 1e-12 * max(np.abs(T).max(), np.abs(V).max()) * np.abs(C).sum(), N
+    N = 2000
+    T, V, C = workloads.make_small_inputs(N, 2, N + 1, seed=4242 + 31 * N + 2, general_V=(N + 2) % 2 == 1)
+    ref, _ = oracle.hc_apply(N, 2, T, V, C)
+    ld = extended.hc_apply_m2_longdouble(N, T, V, C)
+    own = float(np.abs(ref - ld).max())
+    t = 1e-12 * max(np.abs(T).max(), np.abs(V).max()) * np.abs(C).sum()
+    assert own > 0.5 * t                                              # the fp64 oracle itself sits at the north-star bound here
+    assert own <= 8 * 2.0 ** -53 * float(np.abs(ref).max())             # ... while being accurate to a few ulp of max|HC|
