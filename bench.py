@@ -288,6 +288,9 @@ def run_gpu(args):
     barrier, max_over_ranks = job.barrier, job.max_over_ranks
 
     peaks = load_peaks()
+    # FP64 throughput this GPU sustains, measured with register-only kernels (mcb_fp64_peak): plain DFMA chains, DMMA m8n8k4
+    # chains, both interleaved -- the ALU roofline is quoted against the MEASURED figure of the pipe the mode uses
+    fp64_measured = {"dfma_tflops": mcb.fp64_peak(0), "dmma_tflops": mcb.fp64_peak(1), "both_tflops": mcb.fp64_peak(2)}
     R = 3
     c, T, V, Cs = workloads.make_inputs(args.cfg, n_vectors=R)
     sp = mcb.Space(c.N, c.M)
@@ -295,20 +298,45 @@ def run_gpu(args):
     nc, nc1, nc2 = sp.nc, sp.nc_removed(1), sp.nc_removed(2)
     tc = term_counts(c.N, c.M, nc, nc1, nc2)
 
-    # ---- setup (once per space): hashing table, and the maps if the mode needs them ----
-    setup = {}
-    def timed_build(which, name):
+    # ---- setup (once per space): hashing table, and the maps if the mode needs them.  Every builder of the path (Algorithm
+    #      1 / 2 over all nc configurations, hashing table, single- and double-jump map) is timed here,
+    #      as GB/s of the bytes it must move against the measured HBM copy bandwidth: they are HBM-write bound by design ----
+    setup = {"peak_GBps": peaks["hbm_gbs"]}
+    def timed(fn, reps):
+        fn(); torch.cuda.synchronize()
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record(); sp.build_structure(which); b.record(); torch.cuda.synchronize()
-        setup[name + "_ms"] = a.elapsed_time(b)
-        setup[name + "_bytes"] = sp.structure_bytes(which)
-    timed_build(mcb.FOCK_TABLE, "fock_table")
-    timed_build(mcb.FOCK_TABLE, "fock_table")            # second build = warm timing
+        a.record()
+        for _ in range(reps):
+            fn()
+        b.record(); torch.cuda.synchronize()
+        return a.elapsed_time(b) / reps
+    def record(name, ms, nbytes):
+        setup[name] = {"ms": ms, "bytes": nbytes, "GBps": nbytes / (ms * 1e-3) / 1e9, "hbm_frac": nbytes / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"]}
+    fbuf = sp.build_structure(mcb.FOCK_TABLE)
+    record("fock_table", timed(lambda: sp.build_structure(mcb.FOCK_TABLE, buf=fbuf), 5), sp.structure_bytes(mcb.FOCK_TABLE))
     mode = sp.resolve_mode(T, V, MODES[args.mode])       # what MCB_AUTO resolves to for these matrix elements
+    if rank == 0 and not args.no_setup_rates:
+        idx_all = torch.arange(nc, dtype=torch.int32, device="cuda")
+        record("unrank_all", timed(lambda: sp.unrank(idx_all), 5), 4 * (c.M + 1) * nc)
+        occ_all = sp.unrank(idx_all)
+        record("rank_all", timed(lambda: sp.rank(occ_all), 5), 4 * (c.M + 1) * nc)
+        del occ_all, idx_all
+        free, _ = torch.cuda.mem_get_info()
+        for which, name in ((mcb.MAP1, "map1"), (mcb.MAP2, "map2")) + (((mcb.MAP2C, "map2_compact"),) if hasattr(mcb, "MAP2C") and c.N >= 2 else ()):
+            need = sp.structure_bytes(which)
+            if need < 0.6 * free and need < 80e9:
+                mbuf = sp.build_structure(which)
+                record(name, timed(lambda: sp.build_structure(which, buf=mbuf), 3), need + 2 * c.M * nc)     # + the hashing table it reads
+                del mbuf
+                if mode != mcb.MAPS:
+                    sp.drop_structure(which)
+                    torch.cuda.empty_cache()
+            else:
+                setup[name] = {"skipped": f"needs {need / 1e9:.1f} GB (PAPER.md:264: memory is the limit)"}
     map_bytes = 0
     if mode == mcb.MAPS:
-        timed_build(mcb.MAP1, "map1")
-        timed_build(mcb.MAP2, "map2")
+        sp.build_structure(mcb.MAP1)
+        sp.build_structure(mcb.MAP2)
         map_bytes = 4 * nc * (c.M * c.M - c.M) + 4 * nc * tc["P"] ** 2   # entries the kernel may read (upper bound)
 
     dCs = [torch.from_numpy(C).cuda() for C in Cs]
@@ -360,9 +388,14 @@ def run_gpu(args):
     else:
         # contract kernel (GEMM mode) carries every two-body term + the folded one-body terms: 8 flop per packed term
         kflops = 8.0 * tc["two_body_terms_packed"] if mode in (mcb.GEMM, mcb.RUNS) else flops_step
+        pipe = "dmma_tflops" if mode in (mcb.GEMM, mcb.RUNS) else "dfma_tflops"
         roofline = {"bound": "alu", "kernel": KERNELS[mode][dom], "achieved": kflops / (dom_ms * 1e-3) / 1e12,
-                    "peak": alu_peak, "unit": "TFLOP/s",
-                    "peak_source": f"derived: 148 SM x 64 DFMA/clk x 2 x {peaks['sm_max_mhz']:.0f} MHz (DESIGN.md)",
+                    "peak": fp64_measured[pipe], "unit": "TFLOP/s",
+                    "peak_source": f"measured in this run: mcb_fp64_peak, {pipe.split('_')[0].upper()} chains (register-only kernel)",
+                    "peak_measured_tflops": fp64_measured,
+                    "peak_derived_tflops": alu_peak,
+                    "peak_derived_source": f"148 SM x 64 FP64 FMA/clk x 2 x {peaks['sm_max_mhz']:.0f} MHz (DESIGN.md)",
+                    "frac_of_derived": kflops / (dom_ms * 1e-3) / 1e12 / alu_peak,
                     "traffic": None, "algorithmic_flops_per_launch": kflops}
     if (args.cfg, mode) in NCU_TRAFFIC_BYTES:
         roofline["traffic"], roofline["traffic_source"] = NCU_TRAFFIC_BYTES[(args.cfg, mode)]
@@ -437,34 +470,6 @@ def run_gpu(args):
                            "gather_GBps": 16.0 * tc["P"] * nc2 / (rho_ms * 1e-3) / 1e9}
         except Exception as ex:
             line["rho"] = {"error": str(ex)}
-        # hashing and map-build kernels: HBM-write bound by design; GB/s of the bytes they must move
-        try:
-            def timed(fn, reps=5):
-                fn(); torch.cuda.synchronize()
-                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                a.record()
-                for _ in range(reps):
-                    fn()
-                b.record(); torch.cuda.synchronize()
-                return a.elapsed_time(b) / reps
-            hk = {}
-            idx_all = torch.arange(nc, dtype=torch.int32, device="cuda")
-            ms = timed(lambda: sp.unrank(idx_all))
-            hk["unrank_all"] = {"ms": ms, "GBps": 4.0 * (c.M + 1) * nc / (ms * 1e-3) / 1e9}
-            occ_all = sp.unrank(idx_all)
-            ms = timed(lambda: sp.rank(occ_all))
-            hk["rank_all"] = {"ms": ms, "GBps": 4.0 * (c.M + 1) * nc / (ms * 1e-3) / 1e9}
-            del occ_all, idx_all
-            ms = timed(lambda: sp.build_structure(mcb.FOCK_TABLE))
-            hk["fock_table"] = {"ms": ms, "GBps": sp.structure_bytes(mcb.FOCK_TABLE) / (ms * 1e-3) / 1e9}
-            free, _ = torch.cuda.mem_get_info()
-            if sp.structure_bytes(mcb.MAP1) < 0.5 * free:
-                ms = timed(lambda: sp.build_structure(mcb.MAP1), reps=3)
-                hk["map1"] = {"ms": ms, "GBps": sp.structure_bytes(mcb.MAP1) / (ms * 1e-3) / 1e9}
-                sp.drop_structure(mcb.MAP1)
-            line["hash_kernels"] = dict(hk, peak_GBps=peaks["hbm_gbs"])
-        except Exception as ex:
-            line["hash_kernels"] = {"error": str(ex)}
         # Lanczos with full re-orthogonalisation (NEXT-2): 16 steps from C, synchronous API
         try:
             import time
@@ -505,6 +510,7 @@ def main():
     ap.add_argument("--impl", default="mcb", choices=["mcb", "reference"])
     ap.add_argument("--variants", action="store_true", help="also time the other hc_apply modes (short)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-setup-rates", action="store_true", help="skip the timing of the hash / map builders")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     args = ap.parse_args()
     if args.warmup < 3:

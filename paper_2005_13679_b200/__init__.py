@@ -198,11 +198,15 @@ class Space:
             raise McbError(n, "mcb_structure_bytes")
         return n
 
-    def build_structure(self, which: int, stream=None):
-        """Allocate a torch buffer of mcb_structure_bytes and build the structure into it."""
+    def build_structure(self, which: int, stream=None, buf=None):
+        """Build the structure into a torch buffer of mcb_structure_bytes (allocated here unless `buf`, a uint8 CUDA tensor
+        of at least that size, is given -- e.g. to rebuild in place)."""
         torch = _torch()
         nbytes = self.structure_bytes(which)
-        buf = torch.empty(max(nbytes, 256), dtype=torch.uint8, device=self.device)
+        if buf is None:
+            buf = torch.empty(max(nbytes, 256), dtype=torch.uint8, device=self.device)
+        elif buf.dtype != torch.uint8 or not buf.is_cuda or buf.device != self.device or buf.numel() < nbytes or not buf.is_contiguous():
+            raise ValueError("buf must be a contiguous uint8 CUDA tensor of at least structure_bytes on the space's device")
         assert buf.data_ptr() % 256 == 0
         with torch.cuda.device(self.device):
             _check(lib().mcb_build_structure(self._h, which, buf.data_ptr(), nbytes, _stream_ptr(stream)), "mcb_build_structure")

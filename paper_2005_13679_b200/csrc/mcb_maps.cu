@@ -4,7 +4,9 @@
 //   Map1: plane (k*M + l), entry b  =  index of n^(b) - e_k + e_l, or -1 if n_k = 0          (readings A12, A13)
 //   Map2: plane (pair(k<=s)*P + pair(q<=l)), entry b = index of n^(b) - e_k - e_s + e_q + e_l, or -1 if the
 //         removal is not allowed                                                              (reading A15)
-// One thread per configuration b: threads of a warp write consecutive entries of the same plane.
+// One thread per configuration b: threads of a warp write consecutive entries of the same plane.  The occupations come
+// from the hashing table when it is attached (2 M bytes read per configuration against 4 M^2 / 4 P^2 written), otherwise
+// from Algorithm 2 (column searches): with the table the kernels are HBM-write bound.
 #include "mcb_device.cuh"
 
 #define MCB_DISPATCH_M(M, CALL)                                                                          \
@@ -22,15 +24,28 @@
 //   index' = b + sum_{j in [k,l)} (G[j][S_j] - G[j][S_j - 1])      (k < l)
 //   index' = b - sum_{j in [l,k)} (G[j][S_j + 1] - G[j][S_j])      (k > l)
 // i.e. two prefix-sum arrays per configuration and one subtraction per target.
+// prefix sums S_j of configuration b: from the hashing table (occ != NULL) or by Algorithm 2
 template <int MT>
-__global__ void __launch_bounds__(256) k_map1(McbDev d, int* __restrict__ out, long long ld)
+__device__ __forceinline__ void map_prefix(const McbDev& d, const int M, const int b, const uint16_t* __restrict__ occ, const long long ldo, int* S)
+{
+    if (occ != nullptr) {
+        int run = 0;
+#pragma unroll
+        for (int j = 0; j < MTraits<MT>::CAP; ++j) if (j < M) { run += (int)__ldg(occ + (long long)j * ldo + b); S[j] = run; }
+    } else {
+        mcb_unrank_prefix<MT>(d.G, d.ldg, M, d.N, d.nc, b, mcb_top_step(d.N), S);
+    }
+}
+
+template <int MT>
+__global__ void __launch_bounds__(256) k_map1(McbDev d, int* __restrict__ out, long long ld, const uint16_t* __restrict__ occ, long long ldo)
 {
     constexpr int CAP = MTraits<MT>::CAP;
     const int M = MT ? MT : d.M;
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= d.nc) return;
     int S[CAP];
-    mcb_unrank_prefix<MT>(d.G, d.ldg, M, d.N, d.nc, b, mcb_top_step(d.N), S);
+    map_prefix<MT>(d, M, b, occ, ldo, S);
     int PM[CAP], PP[CAP];                  // PM[x] = sum_{j<x} dm[j], PP[x] = sum_{j<x} dp[j]
     int pm = 0, pp = 0;
 #pragma unroll
@@ -66,7 +81,7 @@ __global__ void __launch_bounds__(256) k_map1(McbDev d, int* __restrict__ out, l
 //   index = nc - 1 - X[q] - Y[l],  X[q] = sum_{j<q} (A0[j] - A1[j]),  Y[l] = sum_{j<l} A1[j] + sum_{j>=l} A2[j],
 //   Ai[j] = G[j][S'_j + i].
 template <int MT>
-__global__ void __launch_bounds__(128) k_map2(McbDev d, int* __restrict__ out, long long ld)
+__global__ void __launch_bounds__(128) k_map2(McbDev d, int* __restrict__ out, long long ld, const uint16_t* __restrict__ occ, long long ldo)
 {
     constexpr int CAP = MTraits<MT>::CAP;
     const int M = MT ? MT : d.M;
@@ -74,7 +89,7 @@ __global__ void __launch_bounds__(128) k_map2(McbDev d, int* __restrict__ out, l
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= d.nc) return;
     int S[CAP];
-    mcb_unrank_prefix<MT>(d.G, d.ldg, M, d.N, d.nc, b, mcb_top_step(d.N), S);
+    map_prefix<MT>(d, M, b, occ, ldo, S);
     int a = 0;                                            // removal pair index
     for (int k = 0; k < M; ++k) {
         for (int s = k; s < M; ++s, ++a) {
@@ -132,7 +147,7 @@ int mcb_launch_map1(const mcb_space* sp, int* d_out, long long ld, cudaStream_t 
 {
     const int threads = 256;
     const unsigned blocks = (unsigned)((sp->nc + threads - 1) / threads);
-    MCB_DISPATCH_M(sp->M, (k_map1<MT><<<blocks, threads, 0, st>>>(sp->dev, d_out, ld)));
+    MCB_DISPATCH_M(sp->M, (k_map1<MT><<<blocks, threads, 0, st>>>(sp->dev, d_out, ld, sp->d_fock ? sp->fock.occ : nullptr, sp->fock.ld)));
     MCB_CHECK_LAUNCH();
     return MCB_OK;
 }
@@ -141,7 +156,7 @@ int mcb_launch_map2(const mcb_space* sp, int* d_out, long long ld, cudaStream_t 
 {
     const int threads = 128;
     const unsigned blocks = (unsigned)((sp->nc + threads - 1) / threads);
-    MCB_DISPATCH_M(sp->M, (k_map2<MT><<<blocks, threads, 0, st>>>(sp->dev, d_out, ld)));
+    MCB_DISPATCH_M(sp->M, (k_map2<MT><<<blocks, threads, 0, st>>>(sp->dev, d_out, ld, sp->d_fock ? sp->fock.occ : nullptr, sp->fock.ld)));
     MCB_CHECK_LAUNCH();
     return MCB_OK;
 }

@@ -95,6 +95,18 @@ def test_structures_small(mcb, N, M):
     sp.close()
 
 
+@pytest.mark.parametrize("N,M", [(6, 4), (5, 7), (40, 3), (3, 20), (1, 3)])
+def test_maps_without_hashing_table(mcb, N, M):
+    # the map builders take the occupations from the hashing table when it is attached and from Algorithm 2 otherwise
+    sp = mcb.Space(N, M)
+    sp.build_structure(mcb.MAP1)
+    assert (sp.map1_export(0, sp.nc) == oracle.map1(N, M, 0, sp.nc)).all()
+    if M <= 8:
+        sp.build_structure(mcb.MAP2)
+        assert (sp.map2_export(0, sp.nc) == oracle.map2(N, M, 0, sp.nc)).all()
+    sp.close()
+
+
 @pytest.mark.parametrize("N,M", SMALL)
 @pytest.mark.parametrize("mode", ["REHASH", "MAPS", "GEMM", "RUNS"])
 def test_hc_apply_small(mcb, N, M, mode):
