@@ -328,16 +328,25 @@ def run_gpu(args):
                 mbuf = sp.build_structure(which)
                 record(name, timed(lambda: sp.build_structure(which, buf=mbuf), 3), need + 2 * c.M * nc)     # + the hashing table it reads
                 del mbuf
-                if mode != mcb.MAPS:
-                    sp.drop_structure(which)
-                    torch.cuda.empty_cache()
+                sp.drop_structure(which)
+                torch.cuda.empty_cache()
             else:
                 setup[name] = {"skipped": f"needs {need / 1e9:.1f} GB (PAPER.md:264: memory is the limit)"}
     map_bytes = 0
+    maps_layout = None
     if mode == mcb.MAPS:
-        sp.build_structure(mcb.MAP1)
-        sp.build_structure(mcb.MAP2)
-        map_bytes = 4 * nc * (c.M * c.M - c.M) + 4 * nc * tc["P"] ** 2   # entries the kernel may read (upper bound)
+        # dense planes (the faster layout on this part) when they fit, else the paper's compact double-jump table (T inside V)
+        free, _ = torch.cuda.mem_get_info()
+        dense_fits = sp.structure_bytes(mcb.MAP1) + sp.structure_bytes(mcb.MAP2) < 0.8 * free
+        if c.N >= 2 and (args.compact_maps or not dense_fits):
+            sp.build_structure(mcb.MAP2C)
+            map_bytes = 4 * tc["P"] ** 2 * nc2 + 8 * nc                   # every stride entry + the line offsets
+            maps_layout = "compact (MCB_MAP2C, PAPER.md:212-224)"
+        else:
+            sp.build_structure(mcb.MAP1)
+            sp.build_structure(mcb.MAP2)
+            map_bytes = 4 * nc * (c.M * c.M - c.M) + 4 * nc * tc["P"] ** 2   # entries the kernel may read (upper bound)
+            maps_layout = "dense planes (MCB_MAP1 + MCB_MAP2)"
 
     dCs = [torch.from_numpy(C).cuda() for C in Cs]
     dHCs = [torch.empty_like(d) for d in dCs]
@@ -367,6 +376,10 @@ def run_gpu(args):
 
     # ---- roofline of the dominant kernel ----
     kavg = kms.mean(axis=0) if len(kms) else np.zeros(3)
+    if mode == mcb.MAPS and maps_layout and maps_layout.startswith("compact"):
+        KERNELS[mode] = ["k_hc_maps2c<M>"]
+    if c.M > 12:
+        KERNELS[mode] = ["k_big_gather", "k_big_zgemm", "k_big_reduce"]
     dom = int(np.argmax(kavg))
     dom_ms = float(kavg[dom])
     flops_step = 8.0 * (tc["one_body_terms"] + tc["two_body_terms_packed"])
@@ -412,7 +425,7 @@ def run_gpu(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "complex128 (f64)", "data": "synthetic (seeded, workloads.py)",
-        "config": dict(config_dict(c, MODE_NAMES[mode]),
+        "config": dict(config_dict(c, MODE_NAMES[mode] + (f", {maps_layout}" if maps_layout else "")),
                        l2="inputs larger than L2: 3 rotating C and 3 rotating HC buffers, 16*nc bytes each",
                        replicas="N>1 = independent replicas (path does not shard by north_star)"),
         "applications_per_s": world / (ms_step * 1e-3),
@@ -429,29 +442,38 @@ def run_gpu(args):
     # ---- the other variants, short (map-memory vs recompute trade-off) ----
     if args.variants and rank == 0 and world == 1:
         var = {}
-        for name, m in (("REHASH", mcb.REHASH), ("GEMM", mcb.GEMM), ("RUNS", mcb.RUNS), ("MAPS", mcb.MAPS), ("SPARSE", mcb.SPARSE)):
+        for name, m in (("REHASH", mcb.REHASH), ("GEMM", mcb.GEMM), ("RUNS", mcb.RUNS), ("MAPS_COMPACT", mcb.MAPS), ("MAPS_DENSE", mcb.MAPS),
+                        ("SPARSE", mcb.SPARSE)):
             if m == mcb.SPARSE and sp.resolve_mode(T, V) != mcb.SPARSE:
                 continue
-            if m == mode or (m in (mcb.GEMM, mcb.RUNS) and c.N < 2) or (m == mcb.RUNS and not 2 <= c.M <= 5):
+            if (m == mode and m != mcb.MAPS) or (m in (mcb.GEMM, mcb.RUNS) and c.N < 2) or (m == mcb.RUNS and not 2 <= c.M <= 5):
                 continue
+            if m == mcb.MAPS and (mode == mcb.MAPS or (name == "MAPS_COMPACT" and c.N < 2)):
+                continue
+            built = []
             try:
                 if m == mcb.MAPS:
-                    need = sp.structure_bytes(mcb.MAP1) + sp.structure_bytes(mcb.MAP2)
+                    which = (mcb.MAP2C,) if name == "MAPS_COMPACT" else (mcb.MAP1, mcb.MAP2)
+                    need = sum(sp.structure_bytes(w) for w in which)
                     free, _ = torch.cuda.mem_get_info()
                     if need > 0.8 * free:
                         var[name] = {"skipped": f"maps need {need / 1e9:.1f} GB (PAPER.md:264: memory is the limit)"}
                         continue
-                    sp.build_structure(mcb.MAP1); sp.build_structure(mcb.MAP2)
+                    for w in which:
+                        sp.build_structure(w); built.append(w)
                 ms, km, la = time_mode(sp, mcb, torch, T, V, dCs, dHCs, m, max(3, args.steps // 4), 3, barrier)
                 st = max(3, args.steps // 4)
                 var[name] = {"ms_per_step": ms / st, "configs_per_s": nc / (ms / st * 1e-3)}
                 if m == mcb.MAPS:
-                    mb = 4 * nc * (c.M * c.M - c.M) + 4 * nc * tc["P"] ** 2 + unique_bytes + 2.0 * c.M * nc
-                    var[name]["map_stream_GBps"] = mb / (ms / st * 1e-3) / 1e9
+                    mb = (4 * tc["P"] ** 2 * nc2 + 8 * nc) if name == "MAPS_COMPACT" else (4 * nc * (c.M * c.M - c.M) + 4 * nc * tc["P"] ** 2)
+                    var[name]["map_bytes"] = mb
+                    var[name]["map_stream_GBps"] = (mb + unique_bytes + 2.0 * c.M * nc) / (ms / st * 1e-3) / 1e9
                     var[name]["hbm_frac"] = var[name]["map_stream_GBps"] / peaks["hbm_gbs"]
-                    sp.drop_structure(mcb.MAP1); sp.drop_structure(mcb.MAP2)
             except Exception as ex:  # report, never hide
                 var[name] = {"error": str(ex)}
+            for w in built:
+                sp.drop_structure(w)
+            torch.cuda.empty_cache()
         line["variants"] = var
         # density matrices of the same state: one real SYRK (2P x 2P x nc2) on the DMMA path
         try:
@@ -511,6 +533,7 @@ def main():
     ap.add_argument("--variants", action="store_true", help="also time the other hc_apply modes (short)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-setup-rates", action="store_true", help="skip the timing of the hash / map builders")
+    ap.add_argument("--compact-maps", action="store_true", help="--mode maps: use the paper's compact table (MCB_MAP2C) even where the dense planes fit")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     args = ap.parse_args()
     if args.warmup < 3:

@@ -57,13 +57,19 @@ extern "C" {
                                  (N-2)-particle spaces; needed by every hc_apply mode                         */
 #define MCB_MAP1          1   /* single-jump map                                           */
 #define MCB_MAP2          2   /* double-jump map, dense [pair(k<=s)][pair(q<=l)][b] layout  */
+#define MCB_MAP2C         3   /* double-jump map in the paper's COMPACT layout (Fig. 3): per
+                                 configuration one stride of P targets per ALLOWED removal pair, in the order k = 0..M-1,
+                                 s = k..M-1, behind a per-configuration offset: 4 P^2 nc2 bytes + 8 nc.  Needs
+                                 FOCK_TABLE built first, N >= 2                                                 */
 
 /* hc_apply modes */
 #define MCB_AUTO          0   /* few non-zero elements (at most a quarter of the packed V off its diagonal):
                                  MCB_SPARSE; else N < 2: MCB_REHASH; 2 <= M <= MCB_MAX_M_RUNS and nc >= 2^20:
                                  MCB_RUNS; else MCB_GEMM.  The workspace to provide is that of the dense choice.            */
-#define MCB_MAPS          1   /* per-output gather through the stored Map1 + Map2 (the paper's fastest CPU/GPU
-                                 variant); needs FOCK_TABLE, MAP1, MAP2                      */
+#define MCB_MAPS          1   /* per-output gather through the stored maps (the paper's fastest CPU/GPU variant,
+                                 PAPER.md:238,295).  With the dense planes attached (FOCK_TABLE, MAP1, MAP2): one thread
+                                 per configuration.  Without them but with MAP2C (FOCK_TABLE, MAP2C): a lane group per
+                                 configuration streams its line of the compact table, T riding inside V             */
 #define MCB_REHASH        2   /* per-output gather, target indices recomputed on the fly from the hashing table
                                  ("hashing table + algorithm 1" variant); needs FOCK_TABLE       */
 #define MCB_GEMM          3   /* on-the-fly rehashing, two-body term factored through the (N-2)-particle space:
@@ -128,6 +134,12 @@ int  mcb_detach_structure(mcb_space* sp, int which);
 int  mcb_fock_export(const mcb_space* sp, int removed, long long b0, long long count, int* host_out);
 int  mcb_map1_export(const mcb_space* sp, long long b0, long long count, int* host_out);
 int  mcb_map2_export(const mcb_space* sp, long long b0, long long count, int* host_out);
+/*   map2c: host_offsets int64[count + 1]   stride offset of lines b0 .. b0 + count (line b holds strides
+ *                                           host_offsets[b - b0] .. host_offsets[b - b0 + 1] - 1, one per allowed removal
+ *                                           pair (k <= s) in the paper's order)
+ *          host_entries int32[..][P]        the strides of those lines, P targets (q <= l) each; `capacity` = int32 elements
+ *                                           host_entries can take (MCB_ENOMEM if too small; 0 to fetch the offsets only) */
+int  mcb_map2c_export(const mcb_space* sp, long long b0, long long count, long long* host_offsets, int* host_entries, long long capacity);
 
 /* ---- H.C (Eq. 12) ------------------------------------------------------------------------------------- */
 

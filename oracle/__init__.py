@@ -95,6 +95,48 @@ def map2(N: int, M: int, b0: int, count: int) -> np.ndarray:
     return out
 
 
+def map2_compact(N: int, M: int, b0: int, count: int):
+    """The paper's COMPACT double-jump table (Fig. 3) for lines b0 .. b0 + count - 1, written out as the
+    text says: "for every non-empty IPS k we search for s >= k non-empty as well, and whenever we find such numbers" the
+    line gets one stride with the configurations reached by putting the two particles back -- here the P = M(M+1)/2
+    unordered replacements (q <= l) in pair order (the paper's M^2 stride lists each q != l target twice).  Every target by
+    the literal Algorithm 1 (rank).  Returns (offsets int64 [count + 1], relative to line b0; strides int64 [n, P];
+    pairs int64 [n, 2], the removal (k, s) of every stride)."""
+    P = M * (M + 1) // 2
+    occ = unrank(N, M, np.arange(b0, b0 + count, dtype=np.int64))
+    offsets = [0]
+    removed, pairs = [], []
+    for row in occ:
+        row = row.astype(np.int64)
+        cnt = 0
+        for k in range(M):
+            if row[k] < 1:
+                continue
+            for s in range(k, M):
+                if (s == k and row[k] < 2) or (s != k and row[s] < 1):
+                    continue
+                m = row.copy()
+                m[k] -= 1
+                m[s] -= 1
+                removed.append(m)
+                pairs.append((k, s))
+                cnt += 1
+        offsets.append(offsets[-1] + cnt)
+    n = len(removed)
+    strides = np.empty((n, P), dtype=np.int64)
+    if n:
+        base = np.asarray(removed, dtype=np.int64)
+        c = 0
+        for q in range(M):
+            for l in range(q, M):
+                tgt = base.copy()
+                tgt[:, q] += 1
+                tgt[:, l] += 1
+                strides[:, c] = rank(N, M, tgt)
+                c += 1
+    return np.asarray(offsets, dtype=np.int64), strides, np.asarray(pairs, dtype=np.int64).reshape(n, 2)
+
+
 def hc_apply(N: int, M: int, T: np.ndarray, V: np.ndarray, C: np.ndarray,
              rows: np.ndarray | None = None, nthreads: int = 0):
     """HC restricted to `rows` (all rows if None).  Returns (complex128 [nrows], threads used)."""

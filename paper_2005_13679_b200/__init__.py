@@ -18,14 +18,14 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmcb.so")
 
 OK, EINVAL, ERANGE, ENOMEM, ECUDA, ENOTREADY, EUNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
-FOCK_TABLE, MAP1, MAP2 = 0, 1, 2
+FOCK_TABLE, MAP1, MAP2, MAP2C = 0, 1, 2, 3
 AUTO, MAPS, REHASH, GEMM, RUNS, SPARSE = 0, 1, 2, 3, 4, 5
 MAX_M, MAX_M_APPLY, MAX_M_TILED = 32, 32, 12
 
 EXPORTS = (
     "mcb_space_create", "mcb_space_destroy", "mcb_nc", "mcb_nc_removed", "mcb_binom_table",
     "mcb_unrank", "mcb_rank", "mcb_structure_bytes", "mcb_build_structure", "mcb_detach_structure",
-    "mcb_fock_export", "mcb_map1_export", "mcb_map2_export", "mcb_apply_workspace_bytes",
+    "mcb_fock_export", "mcb_map1_export", "mcb_map2_export", "mcb_map2c_export", "mcb_apply_workspace_bytes",
     "mcb_hc_apply", "mcb_hc_apply_host", "mcb_last_apply_launches", "mcb_timing_enable", "mcb_timing_read", "mcb_fp64_peak", "mcb_strerror", "mcb_last_cuda_error",
     "mcb_rho_workspace_bytes", "mcb_rho", "mcb_lanczos_workspace_bytes", "mcb_lanczos", "mcb_resolve_mode",
     "mcb_lanczos_steps", "mcb_tridiag_eigvals",
@@ -66,6 +66,7 @@ def lib():
         L.mcb_fock_export.argtypes = [vp, i, ll, ll, vp]
         L.mcb_map1_export.argtypes = [vp, ll, ll, vp]
         L.mcb_map2_export.argtypes = [vp, ll, ll, vp]
+        L.mcb_map2c_export.argtypes = [vp, ll, ll, vp, vp, ll]
         L.mcb_apply_workspace_bytes.argtypes = [vp, i]; L.mcb_apply_workspace_bytes.restype = ll
         L.mcb_hc_apply.argtypes = [vp, vp, vp, vp, vp, i, vp, vp]
         L.mcb_hc_apply_host.argtypes = [vp, vp, vp, vp, vp, i, vp, vp, vp, vp]
@@ -232,6 +233,20 @@ class Space:
         out = np.empty((count, self.P, self.P), dtype=np.int32)
         _check(lib().mcb_map2_export(self._h, b0, count, out.ctypes.data), "mcb_map2_export")
         return out
+
+    def map2c_export(self, b0: int, count: int):
+        """(offsets int64 [count + 1], strides int32 [n_strides, P]) of lines b0 .. b0 + count - 1 of the compact double-jump
+        map: line b holds the strides offsets[b - b0] - offsets[0] .. offsets[b - b0 + 1] - offsets[0] - 1 of the second array."""
+        off = np.empty(count + 1, dtype=np.int64)
+        probe = np.empty(1, dtype=np.int32)
+        st = lib().mcb_map2c_export(self._h, b0, count, off.ctypes.data, probe.ctypes.data, 0)
+        if st not in (OK, ENOMEM):
+            raise McbError(st, "mcb_map2c_export")
+        n = int(off[count] - off[0])
+        ent = np.empty((n, self.P), dtype=np.int32)
+        if n > 0:
+            _check(lib().mcb_map2c_export(self._h, b0, count, off.ctypes.data, ent.ctypes.data, n * self.P), "mcb_map2c_export")
+        return off, ent
 
     # -- H.C ----------------------------------------------------------------------------------------------
     def apply_workspace_bytes(self, mode: int = AUTO) -> int:

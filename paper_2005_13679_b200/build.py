@@ -16,7 +16,7 @@ _ROOT = os.path.dirname(_HERE)
 CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(_ROOT, "include")
 LIB = os.path.join(_HERE, "libmcb.so")
-SOURCES = ["mcb_space.cu", "mcb_hash.cu", "mcb_maps.cu", "mcb_apply.cu", "mcb_apply_gemm.cu", "mcb_apply_runs.cu", "mcb_apply_sparse.cu", "mcb_apply_big.cu", "mcb_rho.cu", "mcb_lanczos.cu", "mcb_peak.cu"]
+SOURCES = ["mcb_space.cu", "mcb_hash.cu", "mcb_maps.cu", "mcb_apply.cu", "mcb_apply_gemm.cu", "mcb_apply_runs.cu", "mcb_apply_sparse.cu", "mcb_apply_big.cu", "mcb_map2c.cu", "mcb_rho.cu", "mcb_lanczos.cu", "mcb_peak.cu"]
 HEADERS = [os.path.join(CSRC, "mcb_internal.cuh"), os.path.join(CSRC, "mcb_device.cuh"), os.path.join(INCLUDE, "mcb.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-I" + INCLUDE, "-I" + CSRC] + os.environ.get("MCB_NVCC_EXTRA", "").split()

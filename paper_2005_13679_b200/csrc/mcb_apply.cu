@@ -306,7 +306,11 @@ extern "C" int mcb_hc_apply(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
     if (mode == MCB_SPARSE || (mode == MCB_AUTO && mcb_sparse_preferred(sp, T, V)))
         return mcb_launch_sparse(sp, T, V, d_C, d_HC, st);
     mode = resolve_mode(sp, mode);
-    if (mode == MCB_MAPS && (!sp->d_map1 || (sp->N >= 2 && !sp->d_map2))) return MCB_ENOTREADY;
+    if (mode == MCB_MAPS && (!sp->d_map1 || (sp->N >= 2 && !sp->d_map2))) {
+        // no dense planes: the compact table (T folded into V) serves alone -- one structure, one kernel
+        if (sp->d_map2c && sp->N >= 2) return mcb_launch_maps2c(sp, T, V, d_C, d_HC, st);
+        return MCB_ENOTREADY;
+    }
     if (mode == MCB_RUNS) {
         if (!mcb_runs_supported(sp)) return MCB_EUNSUPPORTED;
         if (!d_workspace || (((uintptr_t)d_workspace) & 255)) return MCB_EINVAL;

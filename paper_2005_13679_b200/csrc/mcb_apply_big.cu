@@ -251,21 +251,7 @@ long long mcb_big_workspace_bytes(const mcb_space* sp)
     return 2 * (long long)sp->P * big_ld2(sp) * (long long)sizeof(double2);
 }
 
-static int big_pair_tables(mcb_space* sp)
-{
-    if (sp->d_pair_ks) return MCB_OK;
-    const int P = sp->P, M = sp->M;
-    unsigned short* h = (unsigned short*)malloc(sizeof(unsigned short) * 2 * (size_t)P);
-    if (!h) return MCB_ENOMEM;
-    int a = 0;
-    for (int k = 0; k < M; ++k)
-        for (int s = k; s < M; ++s, ++a) { h[a] = (unsigned short)k; h[P + a] = (unsigned short)s; }
-    cudaError_t e = cudaMalloc(&sp->d_pair_ks, sizeof(unsigned short) * 2 * (size_t)P);
-    if (e == cudaSuccess) e = cudaMemcpy(sp->d_pair_ks, h, sizeof(unsigned short) * 2 * (size_t)P, cudaMemcpyHostToDevice);
-    free(h);
-    if (e != cudaSuccess) { if (sp->d_pair_ks) { cudaFree(sp->d_pair_ks); sp->d_pair_ks = NULL; } return mcb_set_cuda_error(e); }
-    return MCB_OK;
-}
+static int big_pair_tables(mcb_space* sp) { return mcb_pair_tables(sp); }
 
 static void big_args(const mcb_space* sp, const mcb_c128* d_C, mcb_c128* d_HC, void* d_ws, BigArgs& a)
 {

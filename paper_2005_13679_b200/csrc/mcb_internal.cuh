@@ -42,6 +42,7 @@ struct mcb_space {
     void* d_fock; long long fock_bytes; McbFockView fock;
     int* d_map1;  long long map1_ld;     // [k][l][b], row stride map1_ld
     int* d_map2;  long long map2_ld;     // [ks][ql][b]
+    void* d_map2c;                       // compact double-jump map (mcb_map2c.cu)
     // per-apply staging of packed T, V (device, owned)
     void* d_coef; size_t coef_bytes;
     void* h_coef;              // host scratch for packing
@@ -99,6 +100,13 @@ int mcb_launch_big(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, const mc
 long long mcb_big_rho_workspace_bytes(const mcb_space* sp);
 int mcb_launch_rho_big(mcb_space* sp, const mcb_c128* d_C, mcb_c128* d_rho1, mcb_c128* d_rho2, void* d_ws, cudaStream_t st);
 int mcb_rho_expand_launch(const void* d_G, const mcb_c128* d_C, int N, int M, mcb_c128* d_rho1, mcb_c128* d_rho2, cudaStream_t st);
+
+// compact double-jump map and the MAPS kernel that streams it (mcb_map2c.cu)
+long long mcb_map2c_bytes(const mcb_space* sp);
+int mcb_launch_map2c(mcb_space* sp, void* d_buf, cudaStream_t st);
+int mcb_map2c_export_impl(const mcb_space* sp, long long b0, long long count, long long* host_soff, int* host_entries, long long capacity);
+int mcb_launch_maps2c(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, const mcb_c128* d_C, mcb_c128* d_HC, cudaStream_t st);
+int mcb_pair_tables(mcb_space* sp);
 
 // MCB_SPARSE mode (mcb_apply_sparse.cu)
 bool mcb_sparse_preferred(mcb_space* sp, const mcb_c128* T, const mcb_c128* V);

@@ -176,6 +176,9 @@ extern "C" long long mcb_structure_bytes(const mcb_space* sp, int which)
         return mcb_round_up(sp->nc, 64) * M * M * (long long)sizeof(int);
     case MCB_MAP2:
         return mcb_round_up(sp->nc, 64) * P * P * (long long)sizeof(int);
+    case MCB_MAP2C:
+        if (sp->N < 2) return MCB_EUNSUPPORTED;
+        return mcb_map2c_bytes(sp);
     default:
         return MCB_EINVAL;
     }
@@ -221,6 +224,8 @@ extern "C" int mcb_build_structure(mcb_space* sp, int which, void* d_buf, long l
         sp->d_map2 = (int*)d_buf; sp->map2_ld = ld;
         return MCB_OK;
     }
+    case MCB_MAP2C:
+        return mcb_launch_map2c(sp, d_buf, st);
     default:
         return MCB_EINVAL;
     }
@@ -233,6 +238,7 @@ extern "C" int mcb_detach_structure(mcb_space* sp, int which)
     case MCB_FOCK_TABLE: sp->d_fock = NULL; sp->fock = McbFockView(); return MCB_OK;
     case MCB_MAP1: sp->d_map1 = NULL; return MCB_OK;
     case MCB_MAP2: sp->d_map2 = NULL; return MCB_OK;
+    case MCB_MAP2C: sp->d_map2c = NULL; return MCB_OK;
     default: return MCB_EINVAL;
     }
 }
@@ -279,6 +285,12 @@ extern "C" int mcb_map2_export(const mcb_space* sp, long long b0, long long coun
     if (!sp->d_map2) return MCB_ENOTREADY;
     if (count == 0) return MCB_OK;
     return export_planes(sp->d_map2, sp->map2_ld, sp->P * sp->P, b0, count, host_out);
+}
+
+extern "C" int mcb_map2c_export(const mcb_space* sp, long long b0, long long count, long long* host_offsets, int* host_entries, long long capacity)
+{
+    if (!sp || !host_offsets || count < 0 || b0 < 0 || b0 + count > sp->nc || capacity < 0 || (capacity > 0 && !host_entries)) return MCB_EINVAL;
+    return mcb_map2c_export_impl(sp, b0, count, host_offsets, host_entries, capacity);
 }
 
 extern "C" int mcb_last_apply_launches(const mcb_space* sp) { return sp ? sp->last_launches : -1; }

@@ -86,3 +86,30 @@ def test_map2_against_brute_force(N, M):
                 assert m2[b, a, c] == pos[tuple(u)]
     nc2 = math.comb(N - 2 + M - 1, M - 1) if N >= 2 else 0
     assert total_allowed == P * nc2                              # each (N-2)-config m and pair (k<=s) once
+
+
+def test_compact_double_jump_table_fig3_and_counts(golden_dir):
+    """oracle.map2_compact (the paper's variable-length table) against what the paper fixes: the Fig. 3
+    configuration has 4 strides, and "the transitions that come from removing the last two particles" are 3 strides in
+    (PAPER.md:222); in the paper's M^2-stride count that is 4 x 5^2 = 100 stored targets against 5^4 = 625 (golden file).
+    Against the mathematics: sum over lines of the strides = P nc2; every stride equals the allowed row of the dense table
+    (itself pinned by brute-force particle moves above)."""
+    line = [l for l in open(os.path.join(golden_dir, "paper_fig3_double_jump.txt")) if not l.startswith("#")][0].split()
+    N, M, allowed, stored, naive = map(int, line)
+    occ = np.array([[2, 1, 1, 0, 0]])
+    b = int(oracle.rank(N, M, occ)[0])
+    off, strides, pairs = oracle.map2_compact(N, M, b, 1)
+    assert off.tolist() == [0, allowed] and allowed * M * M == stored and M ** 4 == naive
+    assert pairs.tolist() == [[0, 0], [0, 1], [0, 2], [1, 2]]            # k = 0..M-1, s = k..M-1, allowed ones only
+    assert pairs.tolist().index([1, 2]) == 3                              # "we need to skip 3 strides"
+    for N, M in [(4, 5), (3, 3), (6, 4), (2, 6), (5, 2), (2, 2), (7, 3)]:
+        nc, nc2, P = math.comb(N + M - 1, M - 1), math.comb(N + M - 3, M - 1), M * (M + 1) // 2
+        off, strides, pairs = oracle.map2_compact(N, M, 0, nc)
+        assert off[-1] == P * nc2 == strides.shape[0]
+        dense = oracle.map2(N, M, 0, nc)
+        ok = dense[:, :, 0] >= 0
+        assert (np.diff(off) == ok.sum(axis=1)).all()
+        assert (strides == dense[ok]).all()
+        # a window of the table is the same lines
+        o2, s2, _ = oracle.map2_compact(N, M, nc // 3, nc - nc // 3)
+        assert (o2 + off[nc // 3] == off[nc // 3:]).all() and (s2 == strides[off[nc // 3]:]).all()
