@@ -228,6 +228,12 @@ int  mcb_timing_read(mcb_space* sp, int max_applies, float* ms_out, int* launche
  * *tflops_out (host) receives TFLOP/s.  Allocates and frees 8 bytes of device memory internally. */
 int  mcb_fp64_peak(int kind, double* tflops_out, void* stream);
 
+/* Debug builds only (nvcc -DMCB_DEBUG_BOUNDS): every gather / scatter index of the apply, map and density kernels is
+ * checked against its range on the device.  Synchronises the device and writes host_out[0] = code of the first
+ * violating site since the space was created (0: none), host_out[1] = the offending index.  Returns 1 if the checks are
+ * compiled in, 0 if not (release build: host_out = {0, 0}), or an MCB_E* code. */
+int  mcb_debug_bounds(const mcb_space* sp, long long* host_out);
+
 /* ---- errors ------------------------------------------------------------------------------------------- */
 const char* mcb_strerror(int status);
 int         mcb_last_cuda_error(void);       /* cudaError_t of the last failing CUDA call in this thread */

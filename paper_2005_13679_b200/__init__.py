@@ -28,7 +28,7 @@ EXPORTS = (
     "mcb_fock_export", "mcb_map1_export", "mcb_map2_export", "mcb_map2c_export", "mcb_apply_workspace_bytes",
     "mcb_hc_apply", "mcb_hc_apply_host", "mcb_last_apply_launches", "mcb_timing_enable", "mcb_timing_read", "mcb_fp64_peak", "mcb_strerror", "mcb_last_cuda_error",
     "mcb_rho_workspace_bytes", "mcb_rho", "mcb_lanczos_workspace_bytes", "mcb_lanczos", "mcb_resolve_mode",
-    "mcb_lanczos_steps", "mcb_tridiag_eigvals",
+    "mcb_lanczos_steps", "mcb_tridiag_eigvals", "mcb_debug_bounds",
 )
 
 _lib = None
@@ -79,6 +79,7 @@ def lib():
         L.mcb_rho.argtypes = [vp, vp, vp, vp, vp, vp]
         L.mcb_lanczos_workspace_bytes.argtypes = [vp, i]; L.mcb_lanczos_workspace_bytes.restype = ll
         L.mcb_lanczos.argtypes = [vp, vp, vp, vp, i, i, ctypes.c_double, vp, vp, ctypes.POINTER(i), vp, vp, vp]
+        L.mcb_debug_bounds.argtypes = [vp, vp]
         L.mcb_lanczos_steps.argtypes = [vp, i]
         L.mcb_tridiag_eigvals.argtypes = [i, vp, vp, vp]
         L.mcb_strerror.argtypes = [i]; L.mcb_strerror.restype = ctypes.c_char_p
@@ -377,6 +378,14 @@ class Space:
         if n < 0:
             raise McbError(n, "mcb_timing_read")
         return ms[:n], la[:n]
+
+    def debug_bounds(self):
+        """(compiled_in, site, index): the library's own bounds checks (builds with -DMCB_DEBUG_BOUNDS); site 0 = no violation."""
+        out = np.zeros(2, dtype=np.int64)
+        r = lib().mcb_debug_bounds(self._h, out.ctypes.data)
+        if r < 0:
+            raise McbError(int(r), "mcb_debug_bounds")
+        return bool(r), int(out[0]), int(out[1])
 
     def last_apply_launches(self) -> int:
         return int(lib().mcb_last_apply_launches(self._h))

@@ -135,7 +135,7 @@ __global__ void __launch_bounds__(128) k_hc_direct(DirectArgs p)
                         int tgt;
                         if (USE_MAPS) tgt = __ldg(p.map1 + (long long)(k * M + l) * p.ld1 + g);
                         else tgt = (k < l) ? g + (PM[l] - PM[k]) : g - (PP[k] - PP[l]);
-                        const double2 c = __ldg(p.C + tgt);
+                        const double2 c = __ldg(p.C + MCB_CHK(d, tgt, d.nc, 101));
                         const double f = rk[k] * rl[l];
                         cfma(acc, t, make_double2(f * c.x, f * c.y));
                     }
@@ -193,7 +193,7 @@ __global__ void __launch_bounds__(128) k_hc_direct(DirectArgs p)
 #pragma unroll
                     for (int l = q; l < M; ++l, ++c) {
                         const int tgt = USE_MAPS ? __ldg(m2 + (long long)c * p.ld2) : d.nc - 1 - X[q] - Y[l];
-                        const double2 z = __ldg(p.C + tgt);
+                        const double2 z = __ldg(p.C + MCB_CHK(d, tgt, d.nc, 102));
                         const double f2 = (q == l) ? r2[q] : r1[q] * r1[l];
                         cfma(w, vrow[c], make_double2(f2 * z.x, f2 * z.y));
                     }

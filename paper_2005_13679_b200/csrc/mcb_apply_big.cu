@@ -74,7 +74,7 @@ __global__ void __launch_bounds__(BIG_THREADS) k_big_gather(const BigArgs p)
     int c = 0;
     for (int q = 0; q < M; ++q)
         for (int l = q; l < M; ++l, ++c) {
-            const double2 z = __ldg(p.C + (base - X[q] - Y[l]));
+            const double2 z = __ldg(p.C + MCB_CHK(d, base - X[q] - Y[l], d.nc, 201));
             const double f = (q == l) ? r2[q] : r1[q] * r1[l];
             p.D[(long long)c * p.ld2 + m] = make_double2(f * z.x, f * z.y);
         }
@@ -174,7 +174,7 @@ __global__ void __launch_bounds__(BIG_THREADS) k_big_reduce(const BigArgs p)
         if (n[k] < 1) continue;
         for (int s = k; s < M; ++s) {
             if ((k == s) ? (n[k] < 2) : (n[s] < 1)) continue;
-            const double2 w = p.W[(long long)mcb_pair_index(M, k, s) * p.ld2 + (d.nc2 - 1 - X[k] - Y[s])];
+            const double2 w = p.W[(long long)mcb_pair_index(M, k, s) * p.ld2 + MCB_CHK(d, d.nc2 - 1 - X[k] - Y[s], d.nc2, 202)];
             re += w.x; im += w.y;
         }
     }

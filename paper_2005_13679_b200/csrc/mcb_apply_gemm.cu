@@ -193,7 +193,7 @@ __global__ void __launch_bounds__(GemmCfg<M>::THREADS, GemmCfg<M>::MINB) k_hc2_c
                         for (int l = q; l < M; ++l, ++c) {
                             if (c / (GB * NPARTS) == b && (NPARTS == 1 || (c % NPARTS) == part)) {
                                 const int tgt = d.nc - 1 - X[q] - Y[l];
-                                z[(c % (GB * NPARTS)) / NPARTS] = valid ? __ldg(p.C + tgt) : make_double2(0.0, 0.0);
+                                z[(c % (GB * NPARTS)) / NPARTS] = valid ? __ldg(p.C + MCB_CHK(d, tgt, d.nc, 301)) : make_double2(0.0, 0.0);
                             }
                         }
                     }
@@ -382,7 +382,7 @@ __global__ void __launch_bounds__(256) k_hc2_reduce(GemmArgs p)
         for (int i = 0; i < RB_; ++i) {
             const int a = a0 + i;
             w[i] = make_double2(0.0, 0.0);
-            if (a < P && ok[a]) w[i] = __ldcs(p.W + (size_t)a * p.ldw + mi[a]);
+            if (a < P && ok[a]) w[i] = __ldcs(p.W + (size_t)a * p.ldw + MCB_CHK(d, mi[a], d.nc2, 302));
         }
 #pragma unroll
         for (int i = 0; i < RB_; ++i) { re += w[i].x; im += w[i].y; }

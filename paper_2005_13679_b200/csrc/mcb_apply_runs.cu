@@ -177,17 +177,17 @@ __device__ __forceinline__ void run_prefetch(const RunArgs& p, const int m, cons
         for (int q = 0; q < M; ++q) {
 #pragma unroll
             for (int l = q; l < M; ++l, ++c) {
-                cp_async16(Z + c * Cfg::ZLD, p.C + (valid ? base - X[q] - Y[l] : 0), valid);
+                cp_async16(Z + c * Cfg::ZLD, p.C + (valid ? MCB_CHK(d, base - X[q] - Y[l], d.nc, 401) : 0), valid);
                 F[c * Cfg::FLD] = (q == l) ? r2[q] : r1[q] * r1[l];
             }
         }
     }
-    META[0] = base - X[0] - Y[0];
+    META[0] = valid ? (int)MCB_CHK(d, base - X[0] - Y[0], d.nc, 402) : 0;
 #pragma unroll
     for (int h = 2; h < M; ++h) {
-        META[run_cls_single(h) * 32] = base - X[0] - Y[h];
+        META[run_cls_single(h) * 32] = valid ? (int)MCB_CHK(d, base - X[0] - Y[h], d.nc, 403) : 0;
 #pragma unroll
-        for (int h2 = h; h2 < M; ++h2) META[run_cls_pair<M>(h, h2) * 32] = base - X[h] - Y[h2];
+        for (int h2 = h; h2 < M; ++h2) META[run_cls_pair<M>(h, h2) * 32] = valid ? (int)MCB_CHK(d, base - X[h] - Y[h2], d.nc, 404) : 0;
     }
     META[Cfg::NCLS * 32] = (own ? 1 : 0) | (mj0 == 0 ? 2 : 0) | (mj1 << 2);
 }

@@ -107,7 +107,7 @@ __global__ void __launch_bounds__(128) k_hc_sparse(const SparseArgs p)
                 if (dj != 0) tgt += G0[j] - mcb_ldG(d.G, d.ldg, j, S[j] + dj);
             }
         }
-        const double2 z = __ldg(p.C + tgt);
+        const double2 z = __ldg(p.C + MCB_CHK(p.d, tgt, p.d.nc, 501));
         const double2 v = val[e];
         const double zr = amp * z.x, zi = amp * z.y;
         acc.x = fma(v.x, zr, acc.x); acc.x = fma(-v.y, zi, acc.x);

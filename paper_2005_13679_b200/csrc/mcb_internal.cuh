@@ -22,7 +22,26 @@ struct McbDev {
     const int* G;              // [(M-1)][ldg]   (M == 1: no rows)
     const double* sq;          // sq[j]  = sqrt(j),          j = 0..N+2
     const double* sq2;         // sq2[j] = sqrt(j (j - 1)),  j = 0..N+2   (sq2[0] = sq2[1] = 0)
+    int* dbg;                  // [4] debug words (builds with -DMCB_DEBUG_BOUNDS: first out-of-range index, see MCB_CHK)
 };
+
+// Bounds checks of our own (compute-sanitizer is not available on every pool): in a -DMCB_DEBUG_BOUNDS build every gather
+// and scatter index of the apply / map kernels is checked against its range; the first violation is recorded (site, index)
+// in the space's debug words, the access is redirected to element 0, and mcb_debug_bounds() reports it.  Release builds
+// compile the checks away.
+#ifdef MCB_DEBUG_BOUNDS
+#define MCB_CHK(d, idx, n, site) mcb_chk((d).dbg, (long long)(idx), (long long)(n), (site))
+__device__ __forceinline__ long long mcb_chk(int* dbg, long long idx, long long n, int site)
+{
+    if (idx < 0 || idx >= n) {
+        if (atomicCAS(dbg, 0, site) == 0) { dbg[1] = (int)idx; dbg[2] = (int)(idx >> 32); }
+        return 0;
+    }
+    return idx;
+}
+#else
+#define MCB_CHK(d, idx, n, site) (idx)
+#endif
 
 struct McbFockView {           // hashing table, SoA uint16: occ[j][b], row stride ld
     const uint16_t* occ;       // N-particle space

@@ -149,7 +149,7 @@ __global__ void __launch_bounds__(256) k_m2c_fill(McbDev d, const uint16_t* __re
             }
             __syncwarp(gmask);
             int* dst = entries + stride * P;
-            for (int c = lane; c < P; c += GS) dst[c] = d.nc - 1 - sX[grp][pair_q[c]] - sY[grp][pair_l[c]];
+            for (int c = lane; c < P; c += GS) dst[c] = (int)MCB_CHK(d, d.nc - 1 - sX[grp][pair_q[c]] - sY[grp][pair_l[c]], d.nc, 602);
             ++stride;
         }
     }
@@ -246,7 +246,7 @@ __global__ void __launch_bounds__(M2C_THREADS) k_hc_maps2c(const M2cArgs p)
     };
     auto gather = [&](double2 (&z)[NE], const int (&t)[NE]) {
 #pragma unroll
-        for (int e = 0; e < NE; ++e) z[e] = __ldg(p.C + t[e]);
+        for (int e = 0; e < NE; ++e) z[e] = __ldg(p.C + MCB_CHK(d, t[e], d.nc, 601));
     };
     auto consume = [&](const int r, const double2 (&z)[NE]) {
         const int ks = lst[r];

@@ -113,7 +113,7 @@ __global__ void __launch_bounds__(RhoCfg<M>::THREADS) k_rho_gram(const RhoArgs p
 #pragma unroll
                 for (int l = q; l < M; ++l, ++c) {
                     if (c % Cfg::NPART == part) {
-                        const double2 z = valid ? __ldg(p.C + (d.nc - 1 - X[q] - Y[l])) : make_double2(0.0, 0.0);
+                        const double2 z = valid ? __ldg(p.C + MCB_CHK(d, d.nc - 1 - X[q] - Y[l], d.nc, 701)) : make_double2(0.0, 0.0);
                         const double f = (q == l) ? r2[q] : r1[q] * r1[l];
                         rho_X[(2 * c) * LD + ml] = f * z.x;
                         rho_X[(2 * c + 1) * LD + ml] = f * z.y;

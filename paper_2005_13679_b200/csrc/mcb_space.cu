@@ -76,7 +76,7 @@ extern "C" int mcb_space_create(int N, int M, mcb_space** out)
     size_t g_elems = (size_t)(M > 1 ? M - 1 : 0) * ldg;
     size_t g_bytes = (size_t)mcb_round_up((long long)(g_elems * sizeof(int)), 256);
     size_t sq_bytes = (size_t)mcb_round_up((long long)((N + 3) * sizeof(double)), 256);
-    size_t total = g_bytes + 2 * sq_bytes + 256;
+    size_t total = g_bytes + 2 * sq_bytes + 256;                         // (+ 256: the debug words)
     char* h = (char*)calloc(1, total);
     if (!h) { free(sp->h_binom); delete sp; return MCB_ENOMEM; }
     int* hG = (int*)h;
@@ -109,6 +109,7 @@ extern "C" int mcb_space_create(int N, int M, mcb_space** out)
     sp->dev.G = (const int*)sp->d_consts;
     sp->dev.sq = (const double*)((char*)sp->d_consts + g_bytes);
     sp->dev.sq2 = (const double*)((char*)sp->d_consts + g_bytes + sq_bytes);
+    sp->dev.dbg = (int*)((char*)sp->d_consts + g_bytes + 2 * sq_bytes);  // zero-initialised with the block
     *out = sp;
     return MCB_OK;
 }
@@ -291,6 +292,23 @@ extern "C" int mcb_map2c_export(const mcb_space* sp, long long b0, long long cou
 {
     if (!sp || !host_offsets || count < 0 || b0 < 0 || b0 + count > sp->nc || capacity < 0 || (capacity > 0 && !host_entries)) return MCB_EINVAL;
     return mcb_map2c_export_impl(sp, b0, count, host_offsets, host_entries, capacity);
+}
+
+extern "C" int mcb_debug_bounds(const mcb_space* sp, long long* host_out)
+{
+    if (!sp || !host_out) return MCB_EINVAL;
+    host_out[0] = 0; host_out[1] = 0;
+#ifdef MCB_DEBUG_BOUNDS
+    int w[4] = {0, 0, 0, 0};
+    cudaError_t e = cudaDeviceSynchronize();
+    if (e == cudaSuccess) e = cudaMemcpy(w, sp->dev.dbg, sizeof(w), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return mcb_set_cuda_error(e);
+    host_out[0] = w[0];
+    host_out[1] = ((long long)w[2] << 32) | (unsigned)w[1];
+    return 1;
+#else
+    return 0;
+#endif
 }
 
 extern "C" int mcb_last_apply_launches(const mcb_space* sp) { return sp ? sp->last_launches : -1; }
