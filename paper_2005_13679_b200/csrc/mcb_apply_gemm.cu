@@ -327,8 +327,10 @@ __global__ void __launch_bounds__(GemmCfg<M>::THREADS, GemmCfg<M>::MINB) k_hc2_c
 }
 
 // HC[g] = sum over allowed removal pairs (k<=s) of W'[ks][index2(n^g - e_k - e_s)].  One thread per output.
+// (three or four CTAs per SM: a latency-bound gather lives on resident warps -- left to itself ptxas takes 93 registers at
+// M = 12 and halves them, 1.46 ms against 0.94 ms at configs[4]; measured: M = 10 0.86 ms with three, M = 12 0.94 ms with four)
 template <int M>
-__global__ void __launch_bounds__(256) k_hc2_reduce(GemmArgs p)
+__global__ void __launch_bounds__(256, (M >= 11 ? 4 : 3)) k_hc2_reduce(GemmArgs p)
 {
     const McbDev& d = p.d;
     const int g = blockIdx.x * blockDim.x + threadIdx.x;
