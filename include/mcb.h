@@ -68,7 +68,7 @@ extern "C" {
                                  MCB_RUNS; else MCB_GEMM.  The workspace to provide is that of the dense choice.            */
 #define MCB_MAPS          1   /* per-output gather through the stored maps (the paper's fastest CPU/GPU variant,
                                  PAPER.md:238,295).  With the dense planes attached (FOCK_TABLE, MAP1, MAP2): one thread
-                                 per configuration.  Without them but with MAP2C (FOCK_TABLE, MAP2C): a lane group per
+                                 per configuration.  Without them but with MAP2C (FOCK_TABLE, MAP2C): one thread per
                                  configuration streams its line of the compact table, T riding inside V             */
 #define MCB_REHASH        2   /* per-output gather, target indices recomputed on the fly from the hashing table
                                  ("hashing table + algorithm 1" variant); needs FOCK_TABLE       */

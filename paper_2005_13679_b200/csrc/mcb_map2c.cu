@@ -11,18 +11,29 @@
 //   buffer = [ soff : nc + 1 int64, stride offset of every line (exclusive prefix sum of the allowed-removal counts) ]
 //            [ block sums of the scan ][ entries : P nc2 strides x P int32 ]
 // Build: k_m2c_count (allowed removals per configuration, per-block sums) -> k_m2c_scan (one block scans the block sums)
-//        -> k_m2c_offsets (per-block scan + base) -> k_m2c_fill (a lane group per configuration writes its strides, coalesced).
-// Apply (MCB_MAPS with this map attached): k_hc_maps2c<M> -- a lane group per OUTPUT configuration walks its line stride by
-// stride: coalesced map reads, one C gather per entry, coefficient Vp[a][c] from shared memory (T folded in), amplitude
-// sqrt(n_k (n_s - d_ks)) sqrt((m_q+1)(m_l+1+d_ql)); the group's partial sums are added by shuffles -- no atomics.  The map
-// entries of the NEXT stride are loaded before the gathers of the current one are used, so a gather never waits for the
-// map load in front of it.  This is the paper's own fast variant and the one HBM-bound mode: it streams
-// 4 P^2 nc2 bytes of map per apply.
+//        -> k_m2c_offsets (per-block scan + base) -> k_m2c_fill (one thread per configuration writes its line).
+// Apply (MCB_MAPS with this map attached; T folded into Vp, so the table serves alone):
+//   P <= 15 (M <= 5)  k_hc_maps2c<M>: one thread per OUTPUT configuration, removal pairs walked in lockstep, the next stride of
+//                     the line prefetched into registers before the gathers of the current one (configs[2]: 2.6 ms against
+//                     8.0 ms for the lane-group kernel, 2.3 ms for the dense planes);
+//   P  > 15           k_hc_maps2c_group<M, 32>: a warp per output configuration walks its line stride by stride, one gather per
+//                     lane and stride, partial sums added by shuffles.
+// No atomics anywhere.  This is the paper's own fast variant: it streams 4 P^2 nc2 bytes of map per apply.
 #include <stdlib.h>
 #include <string.h>
 #include "mcb_device.cuh"
 
 #define M2C_BLOCK 1024                // configurations per scan block
+#define MCB_DISPATCH_M(M, CALL)                                                                          \
+    switch (M) {                                                                                         \
+    case 1:  { constexpr int MT = 1;  CALL; } break;  case 2:  { constexpr int MT = 2;  CALL; } break;   \
+    case 3:  { constexpr int MT = 3;  CALL; } break;  case 4:  { constexpr int MT = 4;  CALL; } break;   \
+    case 5:  { constexpr int MT = 5;  CALL; } break;  case 6:  { constexpr int MT = 6;  CALL; } break;   \
+    case 7:  { constexpr int MT = 7;  CALL; } break;  case 8:  { constexpr int MT = 8;  CALL; } break;   \
+    case 9:  { constexpr int MT = 9;  CALL; } break;  case 10: { constexpr int MT = 10; CALL; } break;   \
+    case 11: { constexpr int MT = 11; CALL; } break;  case 12: { constexpr int MT = 12; CALL; } break;   \
+    default: { constexpr int MT = 0;  CALL; } break;                                                     \
+    }
 
 // number of allowed removal pairs of a configuration: (k < s both occupied) + (k == s with n_k >= 2)
 __device__ __forceinline__ int m2c_count(const uint16_t* __restrict__ occ, long long ldo, int M, int g)
@@ -101,56 +112,68 @@ __global__ void __launch_bounds__(256) k_m2c_offsets(McbDev d, const uint16_t* _
     if (blockIdx.x == 0 && threadIdx.x == 0) soff[d.nc] = *total;
 }
 
-// ---- fill: a group of GS lanes per configuration --------------------------------------------------------------------
-// per-group shared scratch: X[M], Y[M] of the current intermediate
-template <int GS>
-__global__ void __launch_bounds__(256) k_m2c_fill(McbDev d, const uint16_t* __restrict__ occ, long long ldo, const long long* __restrict__ soff,
-                                                 const unsigned short* __restrict__ pair_q, const unsigned short* __restrict__ pair_l,
+// ---- fill: one thread per configuration writes its line, stride after stride (the index arithmetic of k_map2, mcb_maps.cu) ----
+// A stride is P consecutive int32 (8-byte aligned when P is even: stored as int2).  The lines of neighbouring threads follow
+// each other in memory, so every sector is completed by the warp within a few strides and leaves L2 once.
+template <int MT>
+__global__ void __launch_bounds__(128) k_m2c_fill(McbDev d, const uint16_t* __restrict__ occ, long long ldo, const long long* __restrict__ soff,
                                                  int* __restrict__ entries)
 {
-    constexpr int GROUPS = 256 / GS;
-    __shared__ int sX[GROUPS][MCB_MAX_M], sY[GROUPS][MCB_MAX_M], sS[GROUPS][MCB_MAX_M];
-    const int M = d.M, P = M * (M + 1) / 2;
-    const int grp = threadIdx.x / GS, lane = threadIdx.x % GS;
-    const long long g_ll = (long long)blockIdx.x * GROUPS + grp;
-    const bool live = g_ll < d.nc;
-    const int g = live ? (int)g_ll : 0;
-    // prefix sums of the configuration (a group never straddles a warp: warp-level barriers order its shared scratch)
-    if (lane == 0) {
+    constexpr int CAP = MTraits<MT>::CAP;
+    const int M = MT ? MT : d.M;
+    const int P = M * (M + 1) / 2;
+    const int g = blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= d.nc) return;
+    int n[CAP], S[CAP];
+    {
         int run = 0;
-        for (int j = 0; j < M; ++j) { run += (int)__ldg(occ + (long long)j * ldo + g); sS[grp][j] = run; }
+#pragma unroll
+        for (int j = 0; j < CAP; ++j) if (j < M) { n[j] = (int)__ldg(occ + (long long)j * ldo + g); run += n[j]; S[j] = run; }
     }
-    __syncwarp();
-    long long stride = live ? soff[g] : 0;
+    int* line = entries + soff[g] * P;
     for (int k = 0; k < M; ++k) {
-        const int nk = sS[grp][k] - (k ? sS[grp][k - 1] : 0);
-        if (!live || nk < 1) continue;                                   // uniform inside the group
         for (int s = k; s < M; ++s) {
-            const int ns = sS[grp][s] - (s ? sS[grp][s - 1] : 0);
-            if ((k == s) ? (nk < 2) : (ns < 1)) continue;
-            // X, Y of the intermediate m = n - e_k - e_s (mcb_maps.cu k_map2): lane j of the group fetches column j
-            const unsigned gmask = GS == 32 ? 0xffffffffu : (((1u << GS) - 1u) << ((threadIdx.x & 31) / GS * GS));
-            __syncwarp(gmask);                                          // the previous stride has been written from sX, sY
-            if (lane == 0) {
-                int x = 0, tot1 = 0;
-                int A1[MCB_MAX_M], A2[MCB_MAX_M];
-                for (int j = 0; j < M; ++j) {
-                    sX[grp][j] = x;
-                    if (j <= M - 2) {
-                        const int sp = sS[grp][j] - (j >= k) - (j >= s);
-                        const int a0 = mcb_ldG(d.G, d.ldg, j, sp);
-                        A1[j] = mcb_ldG(d.G, d.ldg, j, sp + 1);
-                        A2[j] = mcb_ldG(d.G, d.ldg, j, sp + 2);
-                        x += a0 - A1[j]; tot1 += A1[j];
-                    } else { A1[j] = 0; A2[j] = 0; }
-                }
-                int pre = tot1, suf = 0;
-                for (int l = M - 1; l >= 0; --l) { pre -= A1[l]; suf += A2[l]; sY[grp][l] = pre + suf; }
+            int nk = 0, ns = 0;
+#pragma unroll
+            for (int j = 0; j < CAP; ++j) if (j < M) { nk = (j == k) ? n[j] : nk; ns = (j == s) ? n[j] : ns; }
+            if ((k == s) ? (nk < 2) : (nk < 1 || ns < 1)) continue;
+            int X[CAP], Y[CAP], A1[CAP], A2[CAP];
+            int x = 0, tot1 = 0;
+#pragma unroll
+            for (int j = 0; j < CAP; ++j) if (j < M) {
+                X[j] = x;
+                if (j <= M - 2) {
+                    const int sp = S[j] - (j >= k) - (j >= s);
+                    const int a0 = mcb_ldG(d.G, d.ldg, j, sp);
+                    A1[j] = mcb_ldG(d.G, d.ldg, j, sp + 1);
+                    A2[j] = mcb_ldG(d.G, d.ldg, j, sp + 2);
+                    x += a0 - A1[j]; tot1 += A1[j];
+                } else { A1[j] = 0; A2[j] = 0; }
             }
-            __syncwarp(gmask);
-            int* dst = entries + stride * P;
-            for (int c = lane; c < P; c += GS) dst[c] = (int)MCB_CHK(d, d.nc - 1 - sX[grp][pair_q[c]] - sY[grp][pair_l[c]], d.nc, 602);
-            ++stride;
+            int pre = tot1, suf = 0;
+#pragma unroll
+            for (int l = CAP - 1; l >= 0; --l) if (l < M) { pre -= A1[l]; suf += A2[l]; Y[l] = pre + suf; }
+            if (MT != 0 && (MT * (MT + 1) / 2) % 2 == 0) {
+                int2* l2 = reinterpret_cast<int2*>(line);
+                int c = 0, first = 0;
+#pragma unroll
+                for (int q = 0; q < CAP; ++q) if (q < M) {
+#pragma unroll
+                    for (int l = 0; l < CAP; ++l) if (l < M && l >= q) {
+                        const int t = (int)MCB_CHK(d, d.nc - 1 - X[q] - Y[l], d.nc, 602);
+                        if (c & 1) __stcs(l2 + (c >> 1), make_int2(first, t)); else first = t;
+                        ++c;
+                    }
+                }
+            } else {
+                int c = 0;
+#pragma unroll
+                for (int q = 0; q < CAP; ++q) if (q < M) {
+#pragma unroll
+                    for (int l = 0; l < CAP; ++l) if (l < M && l >= q) { __stcs(line + c, (int)MCB_CHK(d, d.nc - 1 - X[q] - Y[l], d.nc, 602)); ++c; }
+                }
+            }
+            line += P;
         }
     }
 }
@@ -164,16 +187,100 @@ struct M2cArgs {
     const double2* Vp;         // [P][P], T folded in (device)
     const long long* soff;
     const int* entries;
+    long long nstrides;        // P nc2 strides in the table
 };
 
-// A group of GS lanes per output configuration g; M2C_THREADS threads per block share one copy of Vp.  Shared memory:
-// Vp [P*P] complex, the sqrt tables, per group the occupations n[M] and the list of its allowed removal pairs.
-#define M2C_THREADS 256
-template <int M, int GS>
+// One thread per output configuration g.  The removal pairs (k <= s) are walked in lockstep by the whole block (uniform
+// coefficient row Vp[a][.] from shared memory, broadcast); a thread whose configuration allows the pair consumes the next
+// stride of its line.  The line is contiguous, so the stride AFTER the current one is loaded before the current one's gathers
+// are issued: no gather waits for the map load in front of it.  Lines of neighbouring threads follow each other in memory:
+// every sector of the table is fetched once from DRAM (L2 holds the few strides a warp is working on).
+#define M2C_THREADS 128
+template <int M>
 __global__ void __launch_bounds__(M2C_THREADS) k_hc_maps2c(const M2cArgs p)
 {
     constexpr int P = M * (M + 1) / 2;
-    constexpr int GROUPS = M2C_THREADS / GS;
+    constexpr bool WIDE = P % 2 == 0;                                    // strides are 8-byte aligned: int2 loads
+    constexpr bool PREFETCH = P <= 15;                                   // two target buffers in registers
+    extern __shared__ double2 m2c_smem[];
+    double2* sV = m2c_smem;                                              // [P*P]
+    const McbDev& d = p.d;
+    for (int i = threadIdx.x; i < P * P; i += M2C_THREADS) sV[i] = p.Vp[i];
+    __syncthreads();
+    const int g = blockIdx.x * M2C_THREADS + threadIdx.x;
+    if (g >= d.nc) return;
+    int n[M];
+#pragma unroll
+    for (int j = 0; j < M; ++j) n[j] = (int)__ldg(p.fock.occ + (long long)j * p.fock.ld + g);
+    const int* line = p.entries + p.soff[g] * (long long)P;
+    const int* const last = p.entries + (p.nstrides - 1) * (long long)P;   // the last stride of the table (prefetch clamp)
+    auto load_stride = [&](int (&t)[P], const int* src) {
+        if (WIDE) {
+#pragma unroll
+            for (int c = 0; c < P; c += 2) { const int2 v = __ldcs(reinterpret_cast<const int2*>(src) + (c >> 1)); t[c] = v.x; t[c + (WIDE ? 1 : 0)] = v.y; }
+        } else {
+#pragma unroll
+            for (int c = 0; c < P; ++c) t[c] = __ldcs(src + c);
+        }
+    };
+    int tcur[P], tnext[PREFETCH ? P : 1];
+    if (PREFETCH) load_stride(tcur, line < last ? line : last);
+    double re = 0.0, im = 0.0;
+#pragma unroll 1
+    for (int k = 0; k < M; ++k) {
+#pragma unroll 1
+        for (int s = k; s < M; ++s) {
+            int nk = 0, ns = 0;
+#pragma unroll
+            for (int j = 0; j < M; ++j) { nk = (j == k) ? n[j] : nk; ns = (j == s) ? n[j] : ns; }
+            const bool ok = (k == s) ? (nk >= 2) : (nk >= 1 && ns >= 1);
+            if (!ok) continue;
+            if (PREFETCH) { const int* nx = line + P; load_stride(reinterpret_cast<int (&)[P]>(tnext), nx < last ? nx : last); }
+            else load_stride(tcur, line);
+            const double f1 = (k == s) ? __ldg(d.sq2 + nk) : __ldg(d.sq + nk) * __ldg(d.sq + ns);
+            double r1[M], r2[M];
+#pragma unroll
+            for (int j = 0; j < M; ++j) {
+                const int mj = n[j] - (j == k) - (j == s);
+                r1[j] = __ldg(d.sq + mj + 1);
+                r2[j] = __ldg(d.sq2 + mj + 2);
+            }
+            const double2* vrow = sV + mcb_pair_index(M, k, s) * P;
+            double wr = 0.0, wi = 0.0;
+            int c = 0;
+#pragma unroll
+            for (int q = 0; q < M; ++q) {
+#pragma unroll
+                for (int l = q; l < M; ++l, ++c) {
+                    const double2 z = __ldg(p.C + MCB_CHK(d, tcur[c], d.nc, 601));
+                    const double f2 = (q == l) ? r2[q] : r1[q] * r1[l];
+                    const double2 v = vrow[c];
+                    const double zr = f2 * z.x, zi = f2 * z.y;
+                    wr = fma(v.x, zr, wr); wr = fma(-v.y, zi, wr);
+                    wi = fma(v.x, zi, wi); wi = fma(v.y, zr, wi);
+                }
+            }
+            re = fma(f1, wr, re); im = fma(f1, wi, im);
+            if (PREFETCH) {
+#pragma unroll
+                for (int cc = 0; cc < P; ++cc) tcur[cc] = tnext[PREFETCH ? cc : 0];
+            }
+            line += P;
+        }
+    }
+    p.HC[g] = make_double2(re, im);
+}
+
+// Many orbitals (P > 15, where a thread cannot keep a stride in registers): a group of GS lanes per output configuration g walks
+// the line stride by stride (coalesced map reads, one gather per lane and stride, partial sums added by shuffles);
+// M2C_GTHREADS threads per persistent block share one copy of Vp.  Shared memory:
+// Vp [P*P] complex, the sqrt tables, per group the occupations n[M] and the list of its allowed removal pairs.
+#define M2C_GTHREADS 256
+template <int M, int GS>
+__global__ void __launch_bounds__(M2C_GTHREADS) k_hc_maps2c_group(const M2cArgs p)
+{
+    constexpr int P = M * (M + 1) / 2;
+    constexpr int GROUPS = M2C_GTHREADS / GS;
     constexpr int NE = (P + GS - 1) / GS;                                // entries of a stride per lane
     extern __shared__ double2 m2c_smem[];
     double2* sV = m2c_smem;                                              // [P*P]
@@ -182,8 +289,8 @@ __global__ void __launch_bounds__(M2C_THREADS) k_hc_maps2c(const M2cArgs p)
     int* sN = reinterpret_cast<int*>(sSq2 + (p.d.N + 3));                // [GROUPS][M]
     unsigned short* sList = reinterpret_cast<unsigned short*>(sN + GROUPS * M);   // [GROUPS][P]: (k << 8) | s of the allowed removals
     const McbDev& d = p.d;
-    for (int i = threadIdx.x; i < P * P; i += M2C_THREADS) sV[i] = p.Vp[i];
-    for (int i = threadIdx.x; i < d.N + 3; i += M2C_THREADS) { sSq[i] = d.sq[i]; sSq2[i] = d.sq2[i]; }
+    for (int i = threadIdx.x; i < P * P; i += M2C_GTHREADS) sV[i] = p.Vp[i];
+    for (int i = threadIdx.x; i < d.N + 3; i += M2C_GTHREADS) { sSq[i] = d.sq[i]; sSq2[i] = d.sq2[i]; }
     const int grp = threadIdx.x / GS, lane = threadIdx.x % GS;
     __syncthreads();                                                     // Vp and the tables are staged ONCE per (persistent) block
     const int* n = sN + grp * M;
@@ -340,15 +447,10 @@ int mcb_launch_map2c(mcb_space* sp, void* d_buf, cudaStream_t st)
     MCB_CHECK_LAUNCH();
     k_m2c_offsets<<<nb, 256, 0, st>>>(sp->dev, sp->fock.occ, sp->fock.ld, bsum, bsum + nb, soff);
     MCB_CHECK_LAUNCH();
-    const int P = sp->P;
-    const unsigned short* pq = sp->d_pair_ks;
-    const unsigned short* pl = sp->d_pair_ks + P;
-    if (P <= 8) {
-        k_m2c_fill<8><<<(unsigned)((sp->nc + 31) / 32), 256, 0, st>>>(sp->dev, sp->fock.occ, sp->fock.ld, soff, pq, pl, entries);
-    } else if (P <= 16) {
-        k_m2c_fill<16><<<(unsigned)((sp->nc + 15) / 16), 256, 0, st>>>(sp->dev, sp->fock.occ, sp->fock.ld, soff, pq, pl, entries);
-    } else {
-        k_m2c_fill<32><<<(unsigned)((sp->nc + 7) / 8), 256, 0, st>>>(sp->dev, sp->fock.occ, sp->fock.ld, soff, pq, pl, entries);
+    {
+        const int threads = 128;
+        const unsigned blocks = (unsigned)((sp->nc + threads - 1) / threads);
+        MCB_DISPATCH_M(sp->M, (k_m2c_fill<MT><<<blocks, threads, 0, st>>>(sp->dev, sp->fock.occ, sp->fock.ld, soff, entries)));
     }
     MCB_CHECK_LAUNCH();
     sp->d_map2c = d_buf;
@@ -374,22 +476,37 @@ int mcb_map2c_export_impl(const mcb_space* sp, long long b0, long long count, lo
     return MCB_OK;
 }
 
-template <int M, int GS>
+template <int M>
 static int launch_maps2c_t(mcb_space* sp, const M2cArgs& a, cudaStream_t st)
 {
     constexpr int P = M * (M + 1) / 2;
-    constexpr int GROUPS = M2C_THREADS / GS;
+    const size_t smem = sizeof(double2) * P * P;
+    if (!(sp->attr_set & (1u << 8))) {
+        MCB_CUDA(cudaFuncSetAttribute(k_hc_maps2c<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        sp->attr_set |= 1u << 8;
+    }
+    const unsigned blocks = (unsigned)((sp->nc + M2C_THREADS - 1) / M2C_THREADS);
+    k_hc_maps2c<M><<<blocks, M2C_THREADS, smem, st>>>(a);
+    MCB_CHECK_LAUNCH();
+    return MCB_OK;
+}
+
+template <int M, int GS>
+static int launch_maps2c_group(mcb_space* sp, const M2cArgs& a, cudaStream_t st)
+{
+    constexpr int P = M * (M + 1) / 2;
+    constexpr int GROUPS = M2C_GTHREADS / GS;
     const size_t smem = sizeof(double2) * P * P + 2 * sizeof(double) * (size_t)(sp->N + 3) + sizeof(int) * GROUPS * M
                         + sizeof(unsigned short) * GROUPS * P + 16;
     if (smem > 227 * 1024) return MCB_EUNSUPPORTED;
-    MCB_CUDA(cudaFuncSetAttribute(k_hc_maps2c<M, GS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    MCB_CUDA(cudaFuncSetAttribute(k_hc_maps2c_group<M, GS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 0, sms = 0;
-    MCB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_hc_maps2c<M, GS>, M2C_THREADS, smem));
+    MCB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_hc_maps2c_group<M, GS>, M2C_GTHREADS, smem));
     MCB_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, sp->device));
     if (per_sm < 1) return MCB_EUNSUPPORTED;
     long long blocks = (sp->nc + GROUPS - 1) / GROUPS;
     if (blocks > (long long)per_sm * sms) blocks = (long long)per_sm * sms;      // persistent: Vp is staged once per block
-    k_hc_maps2c<M, GS><<<(unsigned)blocks, M2C_THREADS, smem, st>>>(a);
+    k_hc_maps2c_group<M, GS><<<(unsigned)blocks, M2C_GTHREADS, smem, st>>>(a);
     MCB_CHECK_LAUNCH();
     return MCB_OK;
 }
@@ -410,20 +527,21 @@ int mcb_launch_maps2c(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, const
     a.C = (const double2*)d_C; a.HC = (double2*)d_HC; a.Vp = (const double2*)sp->d_coef;
     a.soff = (const long long*)sp->d_map2c;
     a.entries = (const int*)((const char*)sp->d_map2c + m2c_soff_bytes(sp) + m2c_bsum_bytes(sp));
+    a.nstrides = (long long)sp->P * sp->nc2;
     { int rc = mcb_tick(sp, 0, st); if (rc) return rc; }
     int rc = MCB_EUNSUPPORTED;
     switch (M) {
-    case 2: rc = launch_maps2c_t<2, 8>(sp, a, st); break;
-    case 3: rc = launch_maps2c_t<3, 8>(sp, a, st); break;
-    case 4: rc = launch_maps2c_t<4, 16>(sp, a, st); break;
-    case 5: rc = launch_maps2c_t<5, 16>(sp, a, st); break;
-    case 6: rc = launch_maps2c_t<6, 32>(sp, a, st); break;
-    case 7: rc = launch_maps2c_t<7, 32>(sp, a, st); break;
-    case 8: rc = launch_maps2c_t<8, 32>(sp, a, st); break;
-    case 9: rc = launch_maps2c_t<9, 32>(sp, a, st); break;
-    case 10: rc = launch_maps2c_t<10, 32>(sp, a, st); break;
-    case 11: rc = launch_maps2c_t<11, 32>(sp, a, st); break;
-    case 12: rc = launch_maps2c_t<12, 32>(sp, a, st); break;
+    case 2: rc = launch_maps2c_t<2>(sp, a, st); break;
+    case 3: rc = launch_maps2c_t<3>(sp, a, st); break;
+    case 4: rc = launch_maps2c_t<4>(sp, a, st); break;
+    case 5: rc = launch_maps2c_t<5>(sp, a, st); break;
+    case 6: rc = launch_maps2c_group<6, 32>(sp, a, st); break;
+    case 7: rc = launch_maps2c_group<7, 32>(sp, a, st); break;
+    case 8: rc = launch_maps2c_group<8, 32>(sp, a, st); break;
+    case 9: rc = launch_maps2c_group<9, 32>(sp, a, st); break;
+    case 10: rc = launch_maps2c_group<10, 32>(sp, a, st); break;
+    case 11: rc = launch_maps2c_group<11, 32>(sp, a, st); break;
+    case 12: rc = launch_maps2c_group<12, 32>(sp, a, st); break;
     default: break;
     }
     if (rc != MCB_OK) return rc;
