@@ -522,6 +522,41 @@ def run_gpu(args):
     return 0
 
 
+def run_sweep(args):
+    """--sweep: the paper's two timing sweeps (M = 3 with N up to 1000; N = 5 with M up to 25), one
+    hc_apply (MCB_AUTO) per point on dense random T, V, C; prints one JSON line.  Context for BASELINE.md, not the metric."""
+    import torch
+    import paper_2005_13679_b200 as mcb
+    pts = [(N, 3) for N in (100, 200, 400, 700, 1000)] + [(5, M) for M in (5, 8, 11, 15, 21, 25)]
+    out = []
+    for N, M in pts:
+        sp = mcb.Space(N, M)
+        T, V, C = workloads.make_small_inputs(N, M, sp.nc, seed=2005 + 13 * N + M)
+        sp.build_structure(mcb.FOCK_TABLE)
+        mode = sp.resolve_mode(T, V)
+        dC = torch.from_numpy(C).cuda()
+        dH = torch.empty_like(dC)
+        for _ in range(max(3, args.warmup)):
+            sp.hc_apply(T, V, dC, out=dH)
+        torch.cuda.synchronize()
+        sp.timing_enable(True)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(args.steps):
+            sp.hc_apply(T, V, dC, out=dH)
+        b.record(); torch.cuda.synchronize()
+        us = 1e3 * a.elapsed_time(b) / args.steps
+        kms, _ = sp.timing_read(min(args.steps, 512))
+        sp.timing_enable(False)
+        k_us = 1e3 * float(kms.sum(axis=1).mean()) if len(kms) else None
+        out.append({"N": N, "M": M, "nc": sp.nc, "mode": MODE_NAMES.get(mode, str(mode)) if M <= 12 else "GEMM (many-orbital path)",
+                    "us_per_apply": us, "kernels_us": k_us, "configs_per_s": sp.nc / (us * 1e-6),
+                    "note": "us_per_apply is back-to-back calls through the Python binding (host-bound below ~50 us); kernels_us = device time of the kernels alone"})
+        sp.close()
+    print(json.dumps({"sweep": "paper shapes (PAPER.md:184,260,289)", "steps": args.steps, "points": out}))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -535,11 +570,14 @@ def main():
     ap.add_argument("--no-setup-rates", action="store_true", help="skip the timing of the hash / map builders")
     ap.add_argument("--compact-maps", action="store_true", help="--mode maps: use the paper's compact table (MCB_MAP2C) even where the dense planes fit")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--sweep", action="store_true", help="time the paper's M = 3 and N = 5 sweeps instead of the metric (one JSON line)")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
     if args.impl == "reference":
         return run_reference(args)
+    if args.sweep:
+        return run_sweep(args)
     return run_gpu(args)
 
 

@@ -259,7 +259,7 @@ static int launch_direct(mcb_space* sp, bool use_maps, const mcb_c128* T, const 
         for (int i = 0; i < P * P; ++i) { h[2 * (M * M + i)] = vr[i]; h[2 * (M * M + i) + 1] = vi[i]; }
     }
     const size_t bytes = sizeof(mcb_c128) * (size_t)(M * M + P * P);
-    MCB_CUDA(cudaMemcpyAsync(sp->d_coef, h, bytes, cudaMemcpyHostToDevice, st));
+    { int rc = mcb_coef_upload(sp, h, bytes, st); if (rc) return rc; }
     DirectArgs a;
     a.d = sp->dev; a.fock = sp->fock;
     a.C = (const double2*)d_C; a.HC = (double2*)d_HC; a.coef = (const double2*)sp->d_coef;

@@ -272,7 +272,7 @@ int mcb_launch_big(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, const mc
         const size_t bytes = sizeof(mcb_c128) * (size_t)M * M;
         if (bytes > sp->coef_bytes) return MCB_ENOMEM;
         memcpy(sp->h_coef, T, bytes);
-        MCB_CUDA(cudaMemcpyAsync(sp->d_coef, sp->h_coef, bytes, cudaMemcpyHostToDevice, st));
+        { int rc = mcb_coef_upload(sp, sp->h_coef, bytes, st); if (rc) return rc; }
         { int rc = mcb_tick(sp, 0, st); if (rc) return rc; }
         k_big_onebody<<<(M + 63) / 64, 64, 0, st>>>((const double2*)sp->d_coef, (const double2*)d_C, (double2*)d_HC, M);
         MCB_CHECK_LAUNCH();
@@ -290,7 +290,7 @@ int mcb_launch_big(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, const mc
     double* vi = vr + pp;
     mcb_pack_pairs(sp->N, M, T, V, true, vr, vi);
     for (size_t i = 0; i < pp; ++i) { h[2 * i] = vr[i]; h[2 * i + 1] = vi[i]; }
-    MCB_CUDA(cudaMemcpyAsync(sp->d_coef, h, sizeof(double) * 2 * pp, cudaMemcpyHostToDevice, st));
+    { int rc = mcb_coef_upload(sp, h, sizeof(double) * 2 * pp, st); if (rc) return rc; }
     BigArgs a;
     big_args(sp, d_C, d_HC, d_ws, a);
     { int rc = mcb_tick(sp, 0, st); if (rc) return rc; }

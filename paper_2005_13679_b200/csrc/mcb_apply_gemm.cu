@@ -439,7 +439,7 @@ static int launch_gemm(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
                 h[mat + (size_t)a * Cfg::A_COLS + c] = im;
             }
         }
-    MCB_CUDA(cudaMemcpyAsync(sp->d_coef, h, a_bytes, cudaMemcpyHostToDevice, st));
+    { int rc = mcb_coef_upload(sp, h, a_bytes, st); if (rc) return rc; }
 
     GemmArgs g;
     g.d = sp->dev; g.fock = sp->fock;

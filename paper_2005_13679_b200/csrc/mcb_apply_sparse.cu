@@ -202,7 +202,7 @@ static int launch_sparse_m(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, 
 {
     int n1, n2; size_t bytes;
     if (sparse_pack(sp, T, V, &n1, &n2, &bytes, false) < 0) return MCB_EUNSUPPORTED;
-    MCB_CUDA(cudaMemcpyAsync(sp->d_coef, sp->h_coef, bytes, cudaMemcpyHostToDevice, st));
+    { int rc = mcb_coef_upload(sp, sp->h_coef, bytes, st); if (rc) return rc; }
     SparseArgs a;
     a.d = sp->dev; a.fock = sp->fock; a.C = (const double2*)d_C; a.HC = (double2*)d_HC;
     a.coef = (const double2*)sp->d_coef; a.n1 = n1; a.n2 = n2;

@@ -22,31 +22,67 @@ __device__ __forceinline__ int hash_rows_here(long long batch, long long base, i
     return (int)(r > threads ? threads : r);
 }
 
+// Algorithm 2: a thread takes UR_SPAN consecutive entries of the batch.  The first is unranked by the column searches; an entry
+// that is the successor of the one before it (idx[i] = idx[i-1] + 1: every entry of an identity-range batch, the common way
+// to list a whole space) is stepped to with the successor rule of the order of Eq. (14) instead (see k_fock_table8) -- one
+// search per UR_SPAN entries; anything else is searched on its own.  Same results either way.
+#define UR_SPAN 4
 template <int MT>
-__global__ void __launch_bounds__(256) k_unrank(McbDev d, const int* __restrict__ idx, long long batch, int* __restrict__ occ, int vec_ok)
+__global__ void __launch_bounds__(256) k_unrank(McbDev d, const int* __restrict__ idx, long long batch, int* __restrict__ occ, int vec_ok, int idx_vec_ok)
 {
     const int M = MT ? MT : d.M;
     const int MP = M | 1;
-    extern __shared__ int s_rows[];                       // [blockDim.x][MP]
-    const long long base = (long long)blockIdx.x * blockDim.x;
-    const long long i = base + threadIdx.x;
+    constexpr int CAP = MTraits<MT>::CAP;
+    extern __shared__ int s_rows[];                       // [blockDim.x * UR_SPAN][MP]
+    const long long base = (long long)blockIdx.x * blockDim.x * UR_SPAN;
+    const long long i0 = base + (long long)threadIdx.x * UR_SPAN;
     const int top = mcb_top_step(d.N);
-    if (i < batch) {
-        int b = idx[i];
-        int S[MTraits<MT>::CAP];
-        int* row = s_rows + threadIdx.x * MP;
-        if (b < 0 || b >= d.nc) {
-#pragma unroll
-            for (int j = 0; j < MTraits<MT>::CAP; ++j) if (j < M) row[j] = -1;
+    if (i0 < batch) {
+        int bb[UR_SPAN];
+        if (idx_vec_ok && i0 + UR_SPAN <= batch) {
+            const int4 q = __ldcs(reinterpret_cast<const int4*>(idx + i0));
+            bb[0] = q.x; bb[1] = q.y; bb[2] = q.z; bb[3] = q.w;
         } else {
-            mcb_unrank_prefix<MT>(d.G, d.ldg, M, d.N, d.nc, b, top, S);
-            int prev = 0;
 #pragma unroll
-            for (int j = 0; j < MTraits<MT>::CAP; ++j) if (j < M) { row[j] = S[j] - prev; prev = S[j]; }
+            for (int e = 0; e < UR_SPAN; ++e) bb[e] = i0 + e < batch ? idx[i0 + e] : -1;
+        }
+        int n[CAP];
+        bool have = false;                                // n holds the configuration of the previous entry
+#pragma unroll
+        for (int e = 0; e < UR_SPAN; ++e) {
+            if (i0 + e >= batch) break;
+            const int b = bb[e];
+            int* row = s_rows + (threadIdx.x * UR_SPAN + e) * MP;
+            if (b < 0 || b >= d.nc) {
+#pragma unroll
+                for (int j = 0; j < CAP; ++j) if (j < M) row[j] = -1;
+                have = false;
+                continue;
+            }
+            if (have && b == bb[e > 0 ? e - 1 : 0] + 1) {
+                if (M >= 2 && n[0] >= 1) { n[0] -= 1; n[1] += 1; }          // inside a run: the common case
+                else {
+                    int S = n[0], jstar = 0;
+#pragma unroll
+                    for (int j = 1; j < CAP; ++j) if (j < M) { if (jstar == 0 && S >= 1) jstar = j; if (jstar == 0) S += n[j]; }
+#pragma unroll
+                    for (int j = 1; j < CAP; ++j) if (j < M) { if (j < jstar) n[j] = 0; else if (j == jstar) n[j] += 1; }
+                    n[0] = S - 1;
+                }
+            } else {
+                int S[CAP];
+                mcb_unrank_prefix<MT>(d.G, d.ldg, M, d.N, d.nc, b, top, S);
+                int prev = 0;
+#pragma unroll
+                for (int j = 0; j < CAP; ++j) if (j < M) { n[j] = S[j] - prev; prev = S[j]; }
+                have = true;
+            }
+#pragma unroll
+            for (int j = 0; j < CAP; ++j) if (j < M) row[j] = n[j];
         }
     }
     __syncthreads();
-    const int total = hash_rows_here(batch, base, blockDim.x) * M;
+    const int total = hash_rows_here(batch, base, blockDim.x * UR_SPAN) * M;
     int* out = occ + base * M;
     const int nvec = vec_ok ? total >> 2 : 0;
     for (int v = threadIdx.x; v < nvec; v += blockDim.x) {
@@ -182,12 +218,16 @@ __global__ void __launch_bounds__(256) k_fock_table8(McbDev d, int Np, int nc_p,
 
 int mcb_launch_unrank(const mcb_space* sp, const int* d_idx, long long batch, int* d_occ, cudaStream_t st)
 {
-    const int threads = 256;
-    const long long blocks = (batch + threads - 1) / threads;
+    const int threads = sp->M <= 12 ? 256 : 64;                          // (rows of a block in shared memory: 4 x threads x (M | 1) ints)
+    const long long per_block = (long long)threads * UR_SPAN;
+    const long long blocks = (batch + per_block - 1) / per_block;
     if (blocks > 2147483647LL) return MCB_ERANGE;
-    const size_t smem = (size_t)threads * (sp->M | 1) * sizeof(int);
-    const int vec_ok = ((uintptr_t)d_occ % 16) == 0;
-    MCB_DISPATCH_M(sp->M, (k_unrank<MT><<<(unsigned)blocks, threads, smem, st>>>(sp->dev, d_idx, batch, d_occ, vec_ok)));
+    const size_t smem = (size_t)per_block * (sp->M | 1) * sizeof(int);
+    const int vec_ok = ((uintptr_t)d_occ % 16) == 0, idx_vec_ok = ((uintptr_t)d_idx % 16) == 0;
+    if (smem > 48 * 1024) {
+        MCB_DISPATCH_M(sp->M, (cudaFuncSetAttribute(k_unrank<MT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)));
+    }
+    MCB_DISPATCH_M(sp->M, (k_unrank<MT><<<(unsigned)blocks, threads, smem, st>>>(sp->dev, d_idx, batch, d_occ, vec_ok, idx_vec_ok)));
     MCB_CHECK_LAUNCH();
     return MCB_OK;
 }

@@ -65,6 +65,9 @@ struct mcb_space {
     // per-apply staging of packed T, V (device, owned)
     void* d_coef; size_t coef_bytes;
     void* h_coef;              // host scratch for packing
+    // pinned ring the packed coefficients are uploaded from (mcb_coef_upload): a pageable source would make every apply
+    // synchronise with the stream; slot i is reused once the copy recorded in ev_pin[i] has completed
+    void* h_pin[4]; cudaEvent_t ev_pin[4]; unsigned pin_next; int pin_state;   // pin_state: 0 not tried, 1 ready, -1 unavailable
     int last_launches;
     // per-space launch state (never process-wide: a process may hold spaces on several devices, used by several threads)
     void* runs_coef;           // host scratch of MCB_RUNS: coefficient matrix + packed Vp (lazily allocated)
@@ -92,6 +95,9 @@ int mcb_set_cuda_error(cudaError_t e);
 
 // ---- pair enumeration (k <= s), order (0,0),(0,1),..,(0,M-1),(1,1),..  (include/mcb.h) ------------------
 __host__ __device__ constexpr int mcb_pair_index(int M, int k, int s) { return k * M - k * (k - 1) / 2 + (s - k); }
+
+// packed T, V of this call -> sp->d_coef, asynchronously on st (mcb_space.cu)
+int mcb_coef_upload(mcb_space* sp, const void* h_src, size_t bytes, cudaStream_t st);
 
 // implemented per translation unit
 int mcb_launch_unrank(const mcb_space* sp, const int* d_idx, long long batch, int* d_occ, cudaStream_t st);

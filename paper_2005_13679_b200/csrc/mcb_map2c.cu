@@ -521,7 +521,7 @@ int mcb_launch_maps2c(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, const
     double* vi = vr + pp;
     mcb_pack_pairs(sp->N, M, T, V, true, vr, vi);                        // T folded in: no single-jump map needed
     for (size_t i = 0; i < pp; ++i) { h[2 * i] = vr[i]; h[2 * i + 1] = vi[i]; }
-    MCB_CUDA(cudaMemcpyAsync(sp->d_coef, h, sizeof(double) * 2 * pp, cudaMemcpyHostToDevice, st));
+    { int rc = mcb_coef_upload(sp, h, sizeof(double) * 2 * pp, st); if (rc) return rc; }
     M2cArgs a;
     a.d = sp->dev; a.fock = sp->fock;
     a.C = (const double2*)d_C; a.HC = (double2*)d_HC; a.Vp = (const double2*)sp->d_coef;

@@ -127,10 +127,36 @@ extern "C" void mcb_space_destroy(mcb_space* sp)
     if (sp->d_consts) cudaFree(sp->d_consts);
     if (sp->d_coef) cudaFree(sp->d_coef);
     if (sp->d_pair_ks) cudaFree(sp->d_pair_ks);
+    for (int i = 0; i < 4; ++i) { if (sp->h_pin[i]) cudaFreeHost(sp->h_pin[i]); if (sp->ev_pin[i]) cudaEventDestroy(sp->ev_pin[i]); }
     free(sp->h_coef);
     free(sp->runs_coef);
     free(sp->h_binom);
     delete sp;
+}
+
+int mcb_coef_upload(mcb_space* sp, const void* h_src, size_t bytes, cudaStream_t st)
+{
+    if (bytes > sp->coef_bytes) return MCB_ENOMEM;
+    if (sp->pin_state == 0) {
+        sp->pin_state = -1;
+        if (sp->coef_bytes <= (1u << 20)) {                              // 4 x coef_bytes of pinned memory (4 x 0.45 MB at M = 12)
+            bool ok = true;
+            for (int i = 0; i < 4 && ok; ++i)
+                ok = cudaHostAlloc(&sp->h_pin[i], sp->coef_bytes, cudaHostAllocDefault) == cudaSuccess
+                     && cudaEventCreateWithFlags(&sp->ev_pin[i], cudaEventDisableTiming) == cudaSuccess;
+            if (ok) sp->pin_state = 1; else (void)cudaGetLastError();
+        }
+    }
+    if (sp->pin_state != 1) {                                            // large M: pageable source (the copy synchronises)
+        MCB_CUDA(cudaMemcpyAsync(sp->d_coef, h_src, bytes, cudaMemcpyHostToDevice, st));
+        return MCB_OK;
+    }
+    const unsigned slot = sp->pin_next++ & 3u;
+    MCB_CUDA(cudaEventSynchronize(sp->ev_pin[slot]));                    // (an event never recorded is complete)
+    memcpy(sp->h_pin[slot], h_src, bytes);
+    MCB_CUDA(cudaMemcpyAsync(sp->d_coef, sp->h_pin[slot], bytes, cudaMemcpyHostToDevice, st));
+    MCB_CUDA(cudaEventRecord(sp->ev_pin[slot], st));
+    return MCB_OK;
 }
 
 extern "C" long long mcb_nc(const mcb_space* sp) { return sp ? sp->nc : -1; }
