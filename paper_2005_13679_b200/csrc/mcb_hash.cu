@@ -101,6 +101,29 @@ __global__ void __launch_bounds__(256) k_rank(McbDev d, const int* __restrict__ 
     const int MP = M | 1;
     extern __shared__ int s_rows[];
     const long long base = (long long)blockIdx.x * blockDim.x;
+    if (MT != 0 && MT % 4 == 0 && vec_ok) {
+        // a row is MT / 4 whole 16-byte vectors: every thread loads its own row (a warp still reads one contiguous block)
+        const long long i = base + threadIdx.x;
+        if (i >= batch) return;
+        const int4* rowv = reinterpret_cast<const int4*>(occ + i * M);
+        int S = 0, acc = 0;
+        bool ok = true;
+#pragma unroll
+        for (int v = 0; v < (MT ? MT : 4) / 4; ++v) {
+            const int4 q = __ldcs(rowv + v);
+            const int x[4] = {q.x, q.y, q.z, q.w};
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const int j = 4 * v + k;
+                ok = ok && x[k] >= 0 && x[k] <= d.N - S;
+                S += ok ? x[k] : 0;
+                if (j <= M - 2) acc += mcb_ldG(d.G, d.ldg, j, S);
+            }
+        }
+        ok = ok && S == d.N;
+        idx[i] = ok ? d.nc - 1 - acc : -1;
+        return;
+    }
     const int total = hash_rows_here(batch, base, blockDim.x) * M;
     const int* in = occ + base * M;
     const int nvec = vec_ok ? total >> 2 : 0;

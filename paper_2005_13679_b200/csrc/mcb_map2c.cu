@@ -450,7 +450,15 @@ int mcb_launch_map2c(mcb_space* sp, void* d_buf, cudaStream_t st)
     {
         const int threads = 128;
         const unsigned blocks = (unsigned)((sp->nc + threads - 1) / threads);
-        MCB_DISPATCH_M(sp->M, (k_m2c_fill<MT><<<blocks, threads, 0, st>>>(sp->dev, sp->fock.occ, sp->fock.ld, soff, entries)));
+        // two blocks per SM (shared memory as the occupancy knob): the partly written sectors of the resident threads' lines
+        // must stay in L2 until the next strides complete them (measured at configs[2]: 6.0 ms with 16 blocks per SM, 4.2 with
+        // 4, 3.0 with 2, 3.6 with 1; configs[4]: 77 / 70 / 60 / 52 ms)
+#ifndef M2C_FILL_BLOCKS_SM
+#define M2C_FILL_BLOCKS_SM 2
+#endif
+        const size_t pad = ((size_t)(220 * 1024) / M2C_FILL_BLOCKS_SM) & ~(size_t)15;
+        MCB_DISPATCH_M(sp->M, (cudaFuncSetAttribute(k_m2c_fill<MT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pad)));
+        MCB_DISPATCH_M(sp->M, (k_m2c_fill<MT><<<blocks, threads, pad, st>>>(sp->dev, sp->fock.occ, sp->fock.ld, soff, entries)));
     }
     MCB_CHECK_LAUNCH();
     sp->d_map2c = d_buf;
