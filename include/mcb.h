@@ -21,7 +21,7 @@
  *   - the library never allocates or frees caller-visible device memory.  The only device memory it owns
  *     is the constants of the mcb_space (binomial / sqrt tables and the staging of the packed T,V: a few hundred KB up to
  *     12 orbitals, 2 x 16 P^2 bytes beyond -- 18 MB at M = 32), allocated in
- *     mcb_space_create and released in mcb_space_destroy (plus, on the first pipelined mcb_hc_apply_host, one copy
+ *     mcb_space_create and released in mcb_space_destroy (plus, on the first pipelined mcb_hc_apply_host, two copy
  *     stream, two events and 64 bytes of pinned host memory).  Hashing table, jump maps and apply workspace
  *     live in caller-provided device buffers (e.g. torch tensors) which must stay alive, unmodified,
  *     for as long as the space uses them.
@@ -167,7 +167,11 @@ int  mcb_resolve_mode(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, int m
  * both vectors are pinned the three steps are PIPELINED: C streams in on a stream owned by the space while the kernel,
  * launched at once on `stream`, waits segment by segment for the prefix of C it needs (an intermediate with top occupation
  * j gathers only inside the first nc - N_c(N-j-3, M) elements), and the trailing sum writes HC straight into the mapped
- * host vector; otherwise copy, apply, copy run one after the other through d_HC_scratch. */
+ * host vector.  When it resolves to MCB_GEMM or MCB_SPARSE (M <= 12, nc >= 2^18, both vectors pinned) the work is cut into
+ * up to 16 slabs by the occupation of the last orbital: a slab's kernels start when the prefix of C it gathers from has
+ * arrived and its piece of HC returns through d_HC_scratch while the next slab computes (two more streams owned by the
+ * space).  Otherwise copy, apply, copy run one after the other through d_HC_scratch.  The results are those of mcb_hc_apply,
+ * bit for bit. */
 int  mcb_hc_apply_host(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
                        const mcb_c128* h_C, mcb_c128* h_HC, int mode,
                        mcb_c128* d_C_scratch, mcb_c128* d_HC_scratch, void* d_workspace, void* stream);

@@ -367,6 +367,91 @@ static int hc_apply_host_pipelined(mcb_space* sp, const mcb_c128* T, const mcb_c
     return MCB_OK;
 }
 
+// Pipelined variant for MCB_GEMM and MCB_SPARSE (M <= MCB_MAX_M_TILED): outputs and intermediates are cut into slabs by the
+// occupation j of the last orbital, the most significant digit of the index order.  An output with n_{M-1} <= j gathers only
+// from configurations with n_{M-1} <= j + 2, a PREFIX of C, and (GEMM) only from intermediates with m_{M-1} <= j; so slab k
+// is computed as soon as its prefix of C is on the device, and its piece of HC goes back to the host while slab k + 1 computes.
+// Three streams: copy-in (pieces of C, one event per slab), the caller's (kernels, waiting on those events), copy-out.
+static int hc_apply_host_slabs(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, const mcb_c128* h_C, mcb_c128* h_HC,
+                               int mode, mcb_c128* d_C, mcb_c128* d_HC, void* d_workspace, cudaStream_t st, bool* done)
+{
+    *done = false;
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, h_C) != cudaSuccess || at.type != cudaMemoryTypeHost) { cudaGetLastError(); return MCB_OK; }
+    if (cudaPointerGetAttributes(&at, h_HC) != cudaSuccess || at.type != cudaMemoryTypeHost) { cudaGetLastError(); return MCB_OK; }
+    if (sp->N < 2 || sp->nc < (1LL << 18)) return MCB_OK;                // too small to be worth three streams
+    if (!sp->copy_stream) {
+        MCB_CUDA(cudaStreamCreateWithFlags(&sp->copy_stream, cudaStreamNonBlocking));
+        MCB_CUDA(cudaEventCreateWithFlags(&sp->ev_a, cudaEventDisableTiming));
+        MCB_CUDA(cudaEventCreateWithFlags(&sp->ev_b, cudaEventDisableTiming));
+        MCB_CUDA(cudaHostAlloc((void**)&sp->h_prog, sizeof(int) * (MCB_H2D_CHUNKS + 4), cudaHostAllocDefault));
+    }
+    if (!sp->out_stream) MCB_CUDA(cudaStreamCreateWithFlags(&sp->out_stream, cudaStreamNonBlocking));
+    if (!sp->slabs_store) {
+        sp->slabs_store = (McbSlabs*)calloc(1, sizeof(McbSlabs));
+        if (!sp->slabs_store) return MCB_ENOMEM;
+        for (int k = 0; k < MCB_MAX_SLABS; ++k) {
+            MCB_CUDA(cudaEventCreateWithFlags(&sp->slabs_store->ev_in[k], cudaEventDisableTiming));
+            MCB_CUDA(cudaEventCreateWithFlags(&sp->slabs_store->ev_out[k], cudaEventDisableTiming));
+        }
+    }
+    McbSlabs* sl = sp->slabs_store;
+    const int N = sp->N, M = sp->M, W = M + 1;
+    // configurations of n particles with last occupation <= j: N_c(n, M) - N_c(n - j - 1, M)
+    auto upto = [&](int n, int j) -> long long {
+        const long long all = sp->h_binom[(size_t)n * W + M];
+        return j >= n ? all : all - sp->h_binom[(size_t)(n - j - 1) * W + M];
+    };
+    // cut points: the smallest j whose outputs reach the next 1/MCB_MAX_SLABS of the space
+    sl->n = 0;
+    long long c_sent = 0;
+    {
+        // the kernels of this call wait for the events: order the copy-in stream behind what the caller's stream holds now
+        MCB_CUDA(cudaEventRecord(sp->ev_a, st));
+        MCB_CUDA(cudaStreamWaitEvent(sp->copy_stream, sp->ev_a, 0));
+        MCB_CUDA(cudaStreamWaitEvent(sp->out_stream, sp->ev_a, 0));
+    }
+    for (int j = 0; j <= N && sl->n < MCB_MAX_SLABS; ++j) {
+        const long long g1 = upto(N, j);
+        const long long prev = sl->n ? sl->g_end[sl->n - 1] : 0;
+        const bool last = g1 >= sp->nc || sl->n == MCB_MAX_SLABS - 1;
+        if (!last && g1 - prev < sp->nc / MCB_MAX_SLABS) continue;
+        const int k = sl->n++;
+        sl->g_end[k] = last ? sp->nc : g1;
+        // intermediates with last occupation <= j, rounded up to whole tiles of every tile size in use (64, 128)
+        long long m1 = last ? sp->nc2 : upto(N - 2, j);
+        m1 = (m1 + 127) / 128 * 128;
+        if (m1 > sp->nc2) m1 = sp->nc2;
+        sl->m_end[k] = m1;
+        // the prefix of C the slab gathers from: last occupation of its last intermediate / output, plus two
+        int jx = j;
+        while (jx < N - 2 && upto(N - 2, jx) < m1) ++jx;
+        long long need = last ? sp->nc : upto(N, jx + 2);
+        if (need > sp->nc) need = sp->nc;
+        if (need > c_sent) {
+            MCB_CUDA(cudaMemcpyAsync(d_C + c_sent, h_C + c_sent, (size_t)(need - c_sent) * sizeof(mcb_c128), cudaMemcpyHostToDevice, sp->copy_stream));
+            c_sent = need;
+        }
+        MCB_CUDA(cudaEventRecord(sl->ev_in[k], sp->copy_stream));
+        if (last) break;
+    }
+    sp->slabs = sl;
+    const int rc = mcb_hc_apply(sp, T, V, d_C, d_HC, mode, d_workspace, (void*)st);
+    sp->slabs = NULL;
+    if (rc != MCB_OK) { cudaStreamSynchronize(sp->copy_stream); cudaStreamSynchronize(st); return rc; }
+    long long g0 = 0;
+    for (int k = 0; k < sl->n; ++k) {
+        MCB_CUDA(cudaStreamWaitEvent(sp->out_stream, sl->ev_out[k], 0));
+        if (sl->g_end[k] > g0)
+            MCB_CUDA(cudaMemcpyAsync(h_HC + g0, d_HC + g0, (size_t)(sl->g_end[k] - g0) * sizeof(mcb_c128), cudaMemcpyDeviceToHost, sp->out_stream));
+        g0 = sl->g_end[k];
+    }
+    MCB_CUDA(cudaStreamSynchronize(sp->out_stream));
+    MCB_CUDA(cudaStreamSynchronize(st));
+    *done = true;
+    return MCB_OK;
+}
+
 extern "C" int mcb_hc_apply_host(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
                                  const mcb_c128* h_C, mcb_c128* h_HC, int mode,
                                  mcb_c128* d_C_scratch, mcb_c128* d_HC_scratch, void* d_workspace, void* stream)
@@ -380,6 +465,15 @@ extern "C" int mcb_hc_apply_host(mcb_space* sp, const mcb_c128* T, const mcb_c12
         int rc = hc_apply_host_pipelined(sp, T, V, h_C, h_HC, d_C_scratch, d_workspace, st, &done);
         if (rc != MCB_OK) return rc;
         if (done) return MCB_OK;                                         // else: vectors not pinned, take the plain path
+    }
+    if (sp->d_fock && sp->M <= MCB_MAX_M_TILED && mode >= MCB_AUTO && mode <= MCB_SPARSE && h_C != h_HC) {
+        const int m = mcb_resolve_mode(sp, T, V, mode);
+        if (m == MCB_GEMM || m == MCB_SPARSE) {
+            bool done = false;
+            int rc = hc_apply_host_slabs(sp, T, V, h_C, h_HC, mode, d_C_scratch, d_HC_scratch, d_workspace, st, &done);
+            if (rc != MCB_OK) return rc;
+            if (done) return MCB_OK;
+        }
     }
     MCB_CUDA(cudaMemcpyAsync(d_C_scratch, h_C, len, cudaMemcpyHostToDevice, st));
     int rc = mcb_hc_apply(sp, T, V, d_C_scratch, d_HC_scratch, mode, d_workspace, stream);

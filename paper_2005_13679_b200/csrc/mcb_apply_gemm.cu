@@ -66,7 +66,8 @@ struct GemmArgs {
     const double* A;           // EMBED: [A_ROWS][A_COLS]; else Vr [A_ROWS][A_COLS] then Vi [A_ROWS][A_COLS]
     double2* W;                // [P][ldw]: W'[a][m] = F(m,a) * sum_c Vp[a][c] F(m,c) C[m + e_q + e_l]
     long long ldw;
-    int ntiles;
+    int tile0, ntiles;         // contract: tiles [tile0, ntiles) of this launch
+    int g0, g1;                // reduce: outputs [g0, g1) of this launch
 };
 
 __device__ __forceinline__ void dmma884(double& c0, double& c1, const double a, const double b)
@@ -136,11 +137,11 @@ __global__ void __launch_bounds__(GemmCfg<M>::THREADS, GemmCfg<M>::MINB) k_hc2_c
         constexpr bool PREF = M <= 10;
         int occ_next[M];
         if (PREF) {
-            const int m0 = blockIdx.x * TM + m_local;
+            const int m0 = (p.tile0 + blockIdx.x) * TM + m_local;
 #pragma unroll
-            for (int j = 0; j < M; ++j) occ_next[j] = (blockIdx.x < p.ntiles && m0 < d.nc2) ? (int)p.fock.occ2[(long long)j * p.fock.ld2 + m0] : 0;
+            for (int j = 0; j < M; ++j) occ_next[j] = (p.tile0 + blockIdx.x < p.ntiles && m0 < d.nc2) ? (int)p.fock.occ2[(long long)j * p.fock.ld2 + m0] : 0;
         }
-        for (int tile = blockIdx.x; tile < p.ntiles; tile += gridDim.x, ++it) {
+        for (int tile = p.tile0 + blockIdx.x; tile < p.ntiles; tile += gridDim.x, ++it) {
             const int s = it % STAGES;
             double* Dr = smem + s * Cfg::STAGE;                  // [DROWS][LD]   (EMBED: rows 0..P-1 real, P..2P-1 imag)
             double* Di = Dr + Cfg::DROWS * LD;                   // [DROWS][LD]   (non-EMBED only)
@@ -251,7 +252,7 @@ __global__ void __launch_bounds__(GemmCfg<M>::THREADS, GemmCfg<M>::MINB) k_hc2_c
     }
 
     int it = 0;
-    for (int tile = blockIdx.x; tile < p.ntiles; tile += gridDim.x, ++it) {
+    for (int tile = p.tile0 + blockIdx.x; tile < p.ntiles; tile += gridDim.x, ++it) {
         const int s = it % STAGES;
         const double* Dr = smem + s * Cfg::STAGE;
         const double* R1 = Dr + Cfg::NPLANES * Cfg::DROWS * LD;
@@ -333,8 +334,8 @@ template <int M>
 __global__ void __launch_bounds__(256, (M >= 11 ? 4 : 3)) k_hc2_reduce(GemmArgs p)
 {
     const McbDev& d = p.d;
-    const int g = blockIdx.x * blockDim.x + threadIdx.x;
-    if (g >= d.nc) return;
+    const int g = p.g0 + blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= p.g1) return;
     int n[M], X[M], Y[M];
     {
         int A1[M], A2[M];
@@ -456,13 +457,42 @@ static int launch_gemm(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
         if (ctas_per_sm < 1) return MCB_EUNSUPPORTED;
         sp->gemm_sms = sm_count; sp->gemm_ctas_per_sm = ctas_per_sm;
     }
+    const int threads = 256;
+    if (sp->slabs) {
+        // pipelined host apply: per slab (cut by the occupation of the last orbital) the contraction of its intermediates, then
+        // the gather of its outputs -- a removal never raises that occupation, so slab k of HC only needs slabs <= k of W'
+        long long g0 = 0, m0 = 0;
+        int launches = 0;
+        for (int k = 0; k < sp->slabs->n; ++k) {
+            const long long g1 = sp->slabs->g_end[k], m1 = sp->slabs->m_end[k];
+            MCB_CUDA(cudaStreamWaitEvent(st, sp->slabs->ev_in[k], 0));
+            if (m1 > m0) {
+                g.tile0 = (int)(m0 / Cfg::TM); g.ntiles = (int)((m1 + Cfg::TM - 1) / Cfg::TM);
+                int grid = sp->gemm_sms * sp->gemm_ctas_per_sm;
+                if (grid > g.ntiles - g.tile0) grid = g.ntiles - g.tile0;
+                k_hc2_contract<M><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(g);
+                MCB_CHECK_LAUNCH();
+                ++launches;
+            }
+            if (g1 > g0) {
+                g.g0 = (int)g0; g.g1 = (int)g1;
+                k_hc2_reduce<M><<<(unsigned)((g1 - g0 + threads - 1) / threads), threads, 0, st>>>(g);
+                MCB_CHECK_LAUNCH();
+                ++launches;
+            }
+            MCB_CUDA(cudaEventRecord(sp->slabs->ev_out[k], st));
+            g0 = g1; m0 = m1;
+        }
+        sp->last_launches = launches;
+        return MCB_OK;
+    }
+    g.tile0 = 0; g.g0 = 0; g.g1 = (int)sp->nc;
     int grid = sp->gemm_sms * sp->gemm_ctas_per_sm;
     if (grid > g.ntiles) grid = g.ntiles;
     { int rc = mcb_tick(sp, 0, st); if (rc) return rc; }
     k_hc2_contract<M><<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(g);
     MCB_CHECK_LAUNCH();
     { int rc = mcb_tick(sp, 1, st); if (rc) return rc; }
-    const int threads = 256;
     k_hc2_reduce<M><<<(unsigned)((sp->nc + threads - 1) / threads), threads, 0, st>>>(g);
     MCB_CHECK_LAUNCH();
     { int rc = mcb_tick(sp, 2, st); if (rc) return rc; }

@@ -27,6 +27,7 @@ struct SparseArgs {
     double2* HC;
     const double2* coef;       // [M] T_kk, [P] Vp diagonal, [n1 + n2] entry values, then (as int) three index words per entry
     int n1, n2;                // off-diagonal entries of T, of the packed V
+    int g0, g1;                // outputs [g0, g1) of this launch
 };
 
 template <int M>
@@ -44,8 +45,8 @@ __global__ void __launch_bounds__(128) k_hc_sparse(const SparseArgs p)
     const int* idx = reinterpret_cast<const int*>(sp_coef + ncoef);
     int* occ_s = reinterpret_cast<int*>(sp_coef + nwords) + threadIdx.x;       // [M][128]: n_j of this thread at occ_s[j * 128]
     const McbDev& d = p.d;
-    const int g = blockIdx.x * blockDim.x + threadIdx.x;
-    const bool live = g < d.nc;
+    const int g = p.g0 + blockIdx.x * blockDim.x + threadIdx.x;
+    const bool live = g < p.g1;
 
     int S[M], G0[M];                                        // prefix sums and G[j][S_j]
     double dre = 0.0, dim = 0.0;
@@ -207,10 +208,28 @@ static int launch_sparse_m(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, 
     a.d = sp->dev; a.fock = sp->fock; a.C = (const double2*)d_C; a.HC = (double2*)d_HC;
     a.coef = (const double2*)sp->d_coef; a.n1 = n1; a.n2 = n2;
     const int threads = 128;
-    const unsigned blocks = (unsigned)((sp->nc + threads - 1) / threads);
-    { int rc = mcb_tick(sp, 0, st); if (rc) return rc; }
     const size_t smem = bytes + sizeof(int) * (size_t)M * 128;          // + the CTA's occupations
     MCB_CUDA(cudaFuncSetAttribute(k_hc_sparse<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (sp->slabs) {
+        // pipelined host apply: one launch per slab of outputs, each behind the arrival of the prefix of C it gathers from
+        long long g0 = 0;
+        for (int k = 0; k < sp->slabs->n; ++k) {
+            const long long g1 = sp->slabs->g_end[k];
+            MCB_CUDA(cudaStreamWaitEvent(st, sp->slabs->ev_in[k], 0));
+            if (g1 > g0) {
+                a.g0 = (int)g0; a.g1 = (int)g1;
+                k_hc_sparse<M><<<(unsigned)((g1 - g0 + threads - 1) / threads), threads, smem, st>>>(a);
+                MCB_CHECK_LAUNCH();
+            }
+            MCB_CUDA(cudaEventRecord(sp->slabs->ev_out[k], st));
+            g0 = g1;
+        }
+        sp->last_launches = sp->slabs->n;
+        return MCB_OK;
+    }
+    const unsigned blocks = (unsigned)((sp->nc + threads - 1) / threads);
+    a.g0 = 0; a.g1 = (int)sp->nc;
+    { int rc = mcb_tick(sp, 0, st); if (rc) return rc; }
     k_hc_sparse<M><<<blocks, threads, smem, st>>>(a);
     MCB_CHECK_LAUNCH();
     { int rc = mcb_tick(sp, 1, st); if (rc) return rc; }

@@ -50,6 +50,18 @@ struct McbFockView {           // hashing table, SoA uint16: occ[j][b], row stri
     long long ld2;
 };
 
+// Pipelined host apply of the per-output / GEMM modes (mcb_hc_apply_host): outputs and intermediates are cut into slabs by
+// the occupation of the last orbital (the most significant digit of the index order): slab k of the outputs only gathers from
+// a PREFIX of C, so its kernels can start when that prefix has arrived and its piece of HC can leave while slab k + 1 computes.
+#define MCB_MAX_SLABS 16
+struct McbSlabs {
+    int n;
+    long long g_end[MCB_MAX_SLABS];      // outputs of slab k: [g_end[k-1], g_end[k])
+    long long m_end[MCB_MAX_SLABS];      // intermediates of slab k: [m_end[k-1], m_end[k]), multiples of 128 (last: nc2)
+    cudaEvent_t ev_in[MCB_MAX_SLABS];    // recorded on the copy-in stream when the prefix of C slab k needs is on the device
+    cudaEvent_t ev_out[MCB_MAX_SLABS];   // recorded on the compute stream when HC of slab k is complete
+};
+
 struct mcb_space {
     int N, M, P;
     int device;
@@ -79,6 +91,9 @@ struct mcb_space {
     cudaStream_t copy_stream;
     cudaEvent_t ev_a, ev_b;
     int* h_prog;               // [MCB_H2D_CHUNKS + 4], pinned; [MCB_H2D_CHUNKS] receives the kernel's error word
+    cudaStream_t out_stream;   // copy-out stream of the slab pipeline
+    McbSlabs* slabs_store;     // events live here (lazily created)
+    const McbSlabs* slabs;     // non-NULL while a pipelined host apply is being enqueued: the launchers cut their work by it
     // optional per-kernel timing (mcb_timing_enable): ring of event tuples, one per apply
     int timing;                          // 0 = off
     int t_count;                         // applies recorded since enable (saturates at MCB_TIMING_RING)

@@ -121,6 +121,14 @@ extern "C" void mcb_space_destroy(mcb_space* sp)
         for (int j = 0; j <= MCB_MAX_APPLY_KERNELS; ++j)
             if (sp->t_ev[i][j]) cudaEventDestroy(sp->t_ev[i][j]);
     if (sp->copy_stream) cudaStreamDestroy(sp->copy_stream);
+    if (sp->out_stream) cudaStreamDestroy(sp->out_stream);
+    if (sp->slabs_store) {
+        for (int k = 0; k < MCB_MAX_SLABS; ++k) {
+            if (sp->slabs_store->ev_in[k]) cudaEventDestroy(sp->slabs_store->ev_in[k]);
+            if (sp->slabs_store->ev_out[k]) cudaEventDestroy(sp->slabs_store->ev_out[k]);
+        }
+        free(sp->slabs_store);
+    }
     if (sp->ev_a) cudaEventDestroy(sp->ev_a);
     if (sp->ev_b) cudaEventDestroy(sp->ev_b);
     if (sp->h_prog) cudaFreeHost(sp->h_prog);
