@@ -22,7 +22,8 @@
  *     is the constants of the mcb_space (binomial / sqrt tables and the staging of the packed T,V: a few hundred KB up to
  *     12 orbitals, 2 x 16 P^2 bytes beyond -- 18 MB at M = 32), allocated in
  *     mcb_space_create and released in mcb_space_destroy (plus, on the first pipelined mcb_hc_apply_host, two copy
- *     stream, two events and 64 bytes of pinned host memory).  Hashing table, jump maps and apply workspace
+ *     streams, up to 34 events and 80 bytes of pinned host memory; and on the first apply up to 2 MB of pinned host memory
+ *     from which the packed T, V are uploaded).  Hashing table, jump maps and apply workspace
  *     live in caller-provided device buffers (e.g. torch tensors) which must stay alive, unmodified,
  *     for as long as the space uses them.
  *   - complex numbers are interleaved (re, im) doubles == C99 double complex == torch.complex128.
