@@ -147,6 +147,12 @@ __global__ void __launch_bounds__(128) k_hc_direct(DirectArgs p)
     // ---- two-body: sum over allowed removal pairs (k<=s), then all insertion pairs (q<=l) ----
     if (d.N >= 2) {
         constexpr int PAIR_UNROLL = CACHE ? M : 1;
+        constexpr bool MAP_PREFETCH = USE_MAPS && P <= 15;               // two target buffers in registers
+        int tcur[MAP_PREFETCH ? P : 1], tnext[MAP_PREFETCH ? P : 1];
+        if (MAP_PREFETCH) {
+#pragma unroll
+            for (int cc = 0; cc < P; ++cc) tnext[MAP_PREFETCH ? cc : 0] = __ldg(p.map2 + (long long)cc * p.ld2 + g);
+        }
         int a_run = 0;                                                   // pair counter of the rolled loops
 #pragma unroll PAIR_UNROLL
         for (int k = 0; k < M; ++k) {
@@ -158,6 +164,18 @@ __global__ void __launch_bounds__(128) k_hc_direct(DirectArgs p)
 #pragma unroll
                 for (int j = 0; j < M; ++j) { nk = (j == k) ? n[j] : nk; ns = (j == s) ? n[j] : ns; }
                 const bool ok = (k == s) ? (nk >= 2) : (nk >= 1 && ns >= 1);
+                if (MAP_PREFETCH) {
+                    // the targets of this pair were loaded one pair ago; those of the next pair (whether it is allowed or not: the
+                    // planes of forbidden removals hold -1) are loaded before this pair's gathers are issued (a second pair of
+                    // look-ahead changes nothing: 1.75 against 1.71 ms at configs[2])
+#pragma unroll
+                    for (int cc = 0; cc < P; ++cc) tcur[cc] = tnext[cc];
+                    if (a + 1 < P) {
+                        const int* m2n = p.map2 + (long long)(a + 1) * P * p.ld2 + g;
+#pragma unroll
+                        for (int cc = 0; cc < P; ++cc) tnext[cc] = __ldg(m2n + (long long)cc * p.ld2);
+                    }
+                }
                 if (!ok) continue;
                 const double f1 = (k == s) ? __ldg(d.sq2 + nk) : __ldg(d.sq + nk) * __ldg(d.sq + ns);
                 double r1[M], r2[M];
@@ -192,7 +210,7 @@ __global__ void __launch_bounds__(128) k_hc_direct(DirectArgs p)
                 for (int q = 0; q < M; ++q) {
 #pragma unroll
                     for (int l = q; l < M; ++l, ++c) {
-                        const int tgt = USE_MAPS ? __ldg(m2 + (long long)c * p.ld2) : d.nc - 1 - X[q] - Y[l];
+                        const int tgt = MAP_PREFETCH ? tcur[c] : (USE_MAPS ? __ldg(m2 + (long long)c * p.ld2) : d.nc - 1 - X[q] - Y[l]);
                         const double2 z = __ldg(p.C + MCB_CHK(d, tgt, d.nc, 102));
                         const double f2 = (q == l) ? r2[q] : r1[q] * r1[l];
                         cfma(w, vrow[c], make_double2(f2 * z.x, f2 * z.y));

@@ -217,10 +217,10 @@ __global__ void __launch_bounds__(M2C_THREADS) k_hc_maps2c(const M2cArgs p)
     auto load_stride = [&](int (&t)[P], const int* src) {
         if (WIDE) {
 #pragma unroll
-            for (int c = 0; c < P; c += 2) { const int2 v = __ldcs(reinterpret_cast<const int2*>(src) + (c >> 1)); t[c] = v.x; t[c + (WIDE ? 1 : 0)] = v.y; }
+            for (int c = 0; c < P; c += 2) { const int2 v = __ldg(reinterpret_cast<const int2*>(src) + (c >> 1)); t[c] = v.x; t[c + (WIDE ? 1 : 0)] = v.y; }
         } else {
 #pragma unroll
-            for (int c = 0; c < P; ++c) t[c] = __ldcs(src + c);
+            for (int c = 0; c < P; ++c) t[c] = __ldg(src + c);
         }
     };
     int tcur[P], tnext[PREFETCH ? P : 1];
