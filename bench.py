@@ -410,7 +410,7 @@ def run_gpu(args):
                     "peak_derived_source": f"148 SM x 64 FP64 FMA/clk x 2 x {peaks['sm_max_mhz']:.0f} MHz (DESIGN.md)",
                     "frac_of_derived": kflops / (dom_ms * 1e-3) / 1e12 / alu_peak,
                     "traffic": None, "algorithmic_flops_per_launch": kflops}
-    if (args.cfg, mode) in NCU_TRAFFIC_BYTES:
+    if (args.cfg, mode) in NCU_TRAFFIC_BYTES and not (mode == mcb.MAPS and maps_layout and maps_layout.startswith("compact")):
         roofline["traffic"], roofline["traffic_source"] = NCU_TRAFFIC_BYTES[(args.cfg, mode)]
         roofline["traffic_unit"] = "bytes per launch (dram read + write, one ncu --set full capture)"
     roofline["frac"] = roofline["achieved"] / roofline["peak"]
