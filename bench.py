@@ -496,7 +496,7 @@ def run_gpu(args):
         try:
             import time
             ksteps = 16
-            sp.lanczos(T, V, dCs[0], 4, mode=mode)
+            sp.lanczos(T, V, dCs[0], ksteps, mode=mode)                  # (same kmax: the basis workspace is allocated here)
             torch.cuda.synchronize(); t0 = time.perf_counter()
             al, be = sp.lanczos(T, V, dCs[0], ksteps, mode=mode)
             torch.cuda.synchronize(); dt = time.perf_counter() - t0
