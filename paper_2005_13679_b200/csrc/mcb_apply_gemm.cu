@@ -40,7 +40,11 @@ template <int M> struct GemmCfg {
     static constexpr int NRB = cdiv(RB, WR);
     static constexpr int WC = WR >= 4 ? 1 : (WR >= 2 ? 2 : 4);
     static constexpr int NWC = WR * WC;                     // consumer warps
-    static constexpr int NWP = (EMBED || M >= 11) ? 4 : 8;  // producer warps (measured: P = 55 wants 8, P = 78 wants 4)
+    // producer warps.  M >= 9: two -- the fewer threads the CTA has, the more registers a consumer warp gets, and with the
+    // 128-register cap of a 448-thread CTA the consumers could not keep the next k-step's fragments in flight (measured at
+    // configs[4], M = 12: contract 4.43 / 4.13 / 3.61 ms with 6 / 4 / 2 producer warps; configs[3], M = 10: 3.72 / 3.81 / 4.12 / 3.67 ms
+    // with 8 / 6 / 4 / 2)
+    static constexpr int NWP = EMBED ? 4 : 2;  // producer warps (measured: P = 55 wants 8, P = 78 wants 4)
     static constexpr int NPT = NWP * 32;                    // producer threads
     static constexpr int TM = EMBED ? 128 : 64;             // intermediates per tile
     static constexpr int LD = TM + 4;                       // smem row stride (doubles): LD % 16 == 4 -> conflict-free B frags
