@@ -38,7 +38,10 @@ template <int M> struct GemmCfg {
     static constexpr int NRB_MAX = cmax(1, 48 / (NK * PER));
     static constexpr int WR = cdiv(RB, NRB_MAX);
     static constexpr int NRB = cdiv(RB, WR);
-    static constexpr int WC = WR >= 4 ? 1 : (WR >= 2 ? 2 : 4);
+    // M = 9, 10: two consumer warps per row block (each sweeps half of the column blocks): 14 DMMA-issuing warps per SM instead
+    // of 7 keep the FP64 tensor pipe fed (configs[3]: contract 3.67 -> 3.40 ms); at M >= 11 the 80 registers of A-fragments per
+    // warp leave no room for that under the 128-register cap of a 512-thread CTA
+    static constexpr int WC = (!EMBED && M <= 10) ? 2 : (WR >= 4 ? 1 : (WR >= 2 ? 2 : 4));
     static constexpr int NWC = WR * WC;                     // consumer warps
     // producer warps.  M >= 9: two -- the fewer threads the CTA has, the more registers a consumer warp gets, and with the
     // 128-register cap of a 448-thread CTA the consumers could not keep the next k-step's fragments in flight (measured at
