@@ -335,10 +335,12 @@ __global__ void __launch_bounds__(GemmCfg<M>::THREADS, GemmCfg<M>::MINB) k_hc2_c
 }
 
 // HC[g] = sum over allowed removal pairs (k<=s) of W'[ks][index2(n^g - e_k - e_s)].  One thread per output.
-// (three or four CTAs per SM: a latency-bound gather lives on resident warps -- left to itself ptxas takes 93 registers at
-// M = 12 and halves them, 1.46 ms against 0.94 ms at configs[4]; measured: M = 10 0.86 ms with three, M = 12 0.94 ms with four)
+// (registers pinned by the launch bounds: a latency-bound gather lives on resident warps -- left to itself ptxas takes 93
+// registers at M = 12 and halves them, 1.46 ms at configs[4].  Measured, configs[3] / configs[4]: 256 threads x 3 | 4 CTAs with 16
+// loads per batch 0.86 / 0.94 ms; 128 threads x 6 | 8 CTAs with 12 | 8 loads per batch 0.80 / 0.88 ms)
+#define RED_T 128
 template <int M>
-__global__ void __launch_bounds__(256, (M >= 11 ? 4 : 3)) k_hc2_reduce(GemmArgs p)
+__global__ void __launch_bounds__(RED_T, (M >= 11 ? 8 : 6)) k_hc2_reduce(GemmArgs p)
 {
     const McbDev& d = p.d;
     const int g = p.g0 + blockIdx.x * blockDim.x + threadIdx.x;
@@ -367,9 +369,7 @@ __global__ void __launch_bounds__(256, (M >= 11 ? 4 : 3)) k_hc2_reduce(GemmArgs 
     // the allowed W' elements are fetched in batches of RB_ loads that are all in flight before the first add
     // (latency-bound gather: run length of the index order is only ~(N+M-1)/(M-1))
     constexpr int P = M * (M + 1) / 2;
-#ifndef REDUCE_BATCH
-#define REDUCE_BATCH 16
-#endif
+    constexpr int REDUCE_BATCH = M >= 11 ? 8 : 12;
     constexpr int RB_ = P <= REDUCE_BATCH ? P : REDUCE_BATCH;
     double re = 0.0, im = 0.0;
     int mi[P];
@@ -464,7 +464,7 @@ static int launch_gemm(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
         if (ctas_per_sm < 1) return MCB_EUNSUPPORTED;
         sp->gemm_sms = sm_count; sp->gemm_ctas_per_sm = ctas_per_sm;
     }
-    const int threads = 256;
+    const int threads = RED_T;
     if (sp->slabs) {
         // pipelined host apply: per slab (cut by the occupation of the last orbital) the contraction of its intermediates, then
         // the gather of its outputs -- a removal never raises that occupation, so slab k of HC only needs slabs <= k of W'
