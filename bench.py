@@ -433,6 +433,9 @@ def run_gpu(args):
         "gflop_per_step": flops_step / 1e9,
         "kernel_ms": {KERNELS[mode][i]: float(kavg[i]) for i in range(len(KERNELS[mode]))},
         "gpu_launches": launches * args.steps,
+        # what each apply enqueues besides its kernels (counted from the launchers, csrc/): one H2D copy of the packed T, V from a
+        # pinned ring (RUNS passes them as a kernel argument instead and clears its tickets / flags with one memset)
+        "gpu_memops_per_step": {"memcpy_h2d": 0 if mode == mcb.RUNS else 1, "memset": 1 if mode == mcb.RUNS else 0},
         "roofline": roofline, "hbm_unique": hbm_unique, "setup": setup, "clocks": clk,
         "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms, "steps": e2e_steps,
                 "h2d_bytes_per_step": 16 * nc + 16 * (c.M ** 2 + c.M ** 4), "d2h_bytes_per_step": 16 * nc,
