@@ -45,6 +45,7 @@ extern "C" {
 #define MCB_ECUDA        -4   /* a CUDA runtime call failed; see mcb_last_cuda_error()                       */
 #define MCB_ENOTREADY    -5   /* a structure the call needs (hashing table, map) has not been built          */
 #define MCB_EUNSUPPORTED -6   /* mode not available for this space (see the hc_apply modes)                    */
+#define MCB_ESCRATCH     -7   /* mcb_rho_static: the problem does not fit the library's fixed scratch array (M too large) */
 
 #define MCB_MAX_M        32   /* hashing and map kernels                                                      */
 #define MCB_MAX_M_APPLY  32   /* hc_apply, rho, lanczos.  Up to 12 orbitals the packed V (P x P complex, P = M(M+1)/2)
@@ -188,6 +189,31 @@ int  mcb_hc_apply_host(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
  * `stream`; all pointers 16-byte aligned. */
 long long mcb_rho_workspace_bytes(const mcb_space* sp);
 int  mcb_rho(mcb_space* sp, const mcb_c128* d_C, mcb_c128* d_rho1, mcb_c128* d_rho2, void* d_workspace, void* stream);
+
+/* The same density matrices (Eq. 10-11) for callers that CANNOT ALLOCATE device memory, hence cannot give
+ * mcb_rho its workspace: a plug-in that receives C and the result buffers from a host program and has no allocator of its
+ * own; a job whose pool claimed the whole device at start-up, so that any further cudaMalloc fails or breaks its memory
+ * budget; a time-stepping loop where cudaMalloc / cudaFree are banned because they synchronise the device and block the
+ * other streams and threads of the process.  The caller passes the input and the two outputs only; the scratch of the
+ * kernels (per-block partial Gram matrices and the reduced P x P matrix) sits in a fixed array of MCB_RHO_STATIC_BYTES
+ * inside the library image.  That array costs its size on EVERY GPU that loads libmcb.so, from the first use of the
+ * density kernels until the process exits, whether or not this call is ever made.
+ *   Limit: M <= MCB_RHO_STATIC_MAX_M (any N the space allows); a larger M returns MCB_ESCRATCH and touches nothing.  When
+ *     the array holds fewer partials than mcb_rho's grid has blocks (M = 3..5 and M >= 8) fewer blocks share the work: same
+ *     result up to summation order (within the tolerance stated for mcb_rho, bit-identical where the grids agree), slower.
+ *   The call itself runs no cudaMalloc / cudaFree / allocating library routine and needs FOCK_TABLE if N >= 2, like mcb_rho.
+ *     (mcb_space_create and the FOCK_TABLE buffer are set-up: do them where allocating is still allowed.)
+ *   First call on a device: looks up the device address of the array (cudaGetSymbolAddress, which also makes the CUDA
+ *     runtime load the kernels' module) and remembers it for that device.  Make that first call during set-up, before any
+ *     stream capture is begun.  The space's device must be the current device (MCB_EINVAL otherwise).
+ *   Sharing: all spaces, streams and threads of the process use the ONE array of a device.  It keeps the previous call's
+ *     contents; nothing needs clearing because each call overwrites every word it later reads.  Two calls whose kernels may
+ *     run at the same time on one GPU (different streams, or different host threads) race on it and give wrong results:
+ *     order them on one stream or with events.  mcb_rho with caller workspaces has no such restriction.
+ * Asynchronous on `stream`; pointers as for mcb_rho. */
+#define MCB_RHO_STATIC_MAX_M   12
+#define MCB_RHO_STATIC_BYTES   (8 << 20)
+int  mcb_rho_static(mcb_space* sp, const mcb_c128* d_C, mcb_c128* d_rho1, mcb_c128* d_rho2, void* stream);
 
 /* ---- Lanczos tridiagonalisation with full re-orthogonalisation -------------------------------
  * Builds, from the start vector d_v0 (device, nc complex, any non-zero norm), the Krylov basis v_0 .. v_k of H in

@@ -17,10 +17,11 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmcb.so")
 
-OK, EINVAL, ERANGE, ENOMEM, ECUDA, ENOTREADY, EUNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
+OK, EINVAL, ERANGE, ENOMEM, ECUDA, ENOTREADY, EUNSUPPORTED, ESCRATCH = 0, -1, -2, -3, -4, -5, -6, -7
 FOCK_TABLE, MAP1, MAP2, MAP2C = 0, 1, 2, 3
 AUTO, MAPS, REHASH, GEMM, RUNS, SPARSE = 0, 1, 2, 3, 4, 5
 MAX_M, MAX_M_APPLY, MAX_M_TILED = 32, 32, 12
+RHO_STATIC_MAX_M, RHO_STATIC_BYTES = 12, 8 << 20
 
 EXPORTS = (
     "mcb_space_create", "mcb_space_destroy", "mcb_nc", "mcb_nc_removed", "mcb_binom_table",
@@ -28,7 +29,7 @@ EXPORTS = (
     "mcb_fock_export", "mcb_map1_export", "mcb_map2_export", "mcb_map2c_export", "mcb_apply_workspace_bytes",
     "mcb_hc_apply", "mcb_hc_apply_host", "mcb_last_apply_launches", "mcb_timing_enable", "mcb_timing_read", "mcb_fp64_peak", "mcb_strerror", "mcb_last_cuda_error",
     "mcb_rho_workspace_bytes", "mcb_rho", "mcb_lanczos_workspace_bytes", "mcb_lanczos", "mcb_resolve_mode",
-    "mcb_lanczos_steps", "mcb_tridiag_eigvals", "mcb_debug_bounds",
+    "mcb_lanczos_steps", "mcb_tridiag_eigvals", "mcb_debug_bounds", "mcb_rho_static",
 )
 
 _lib = None
@@ -77,6 +78,7 @@ def lib():
         L.mcb_resolve_mode.argtypes = [vp, vp, vp, i]
         L.mcb_rho_workspace_bytes.argtypes = [vp]; L.mcb_rho_workspace_bytes.restype = ll
         L.mcb_rho.argtypes = [vp, vp, vp, vp, vp, vp]
+        L.mcb_rho_static.argtypes = [vp, vp, vp, vp, vp]
         L.mcb_lanczos_workspace_bytes.argtypes = [vp, i]; L.mcb_lanczos_workspace_bytes.restype = ll
         L.mcb_lanczos.argtypes = [vp, vp, vp, vp, i, i, ctypes.c_double, vp, vp, ctypes.POINTER(i), vp, vp, vp]
         L.mcb_debug_bounds.argtypes = [vp, vp]
@@ -336,6 +338,29 @@ class Space:
         with torch.cuda.device(self.device):
             _check(lib().mcb_rho(self._h, C.data_ptr(), r1.data_ptr(), r2.data_ptr(), ws.data_ptr(), _stream_ptr(stream)), "mcb_rho")
         return r1, r2
+
+    def rho_static(self, C, rho1=None, rho2=None, stream=None):
+        """mcb_rho_static: the density matrices of `rho` for callers that cannot allocate device memory -- code that is
+        handed its buffers by a host program, runs under a pool that already owns the whole device, or sits in a loop where
+        cudaMalloc's device-wide synchronisation is not acceptable.  No workspace is passed: the kernels' scratch is a fixed
+        8 MiB array inside libmcb.so (M <= RHO_STATIC_MAX_M = 12; McbError with status ESCRATCH beyond).  Pass `rho1` [M,M] and
+        `rho2` [M,M,M,M] (contiguous complex128 CUDA tensors) to keep this Python layer from allocating too; they are created
+        here only when left out.  The first call on a device does a one-time address look-up: make it during set-up.  All
+        calls on a device share the array -- keep them ordered on one stream (overlapping calls race)."""
+        torch = _torch()
+        self._check_vec(C, "C")
+        outs = []
+        for t, shape, name in ((rho1, (self.M, self.M), "rho1"), (rho2, (self.M,) * 4, "rho2")):
+            if t is None:
+                t = torch.empty(shape, dtype=torch.complex128, device=self.device)
+            elif (not isinstance(t, torch.Tensor) or t.dtype != torch.complex128 or not t.is_cuda or not t.is_contiguous()
+                    or tuple(t.shape) != shape or t.device != self.device):
+                raise ValueError(f"{name} must be a contiguous complex128 CUDA tensor of shape {shape} on {self.device}")
+            outs.append(t)
+        with torch.cuda.device(self.device):
+            _check(lib().mcb_rho_static(self._h, C.data_ptr(), outs[0].data_ptr(), outs[1].data_ptr(), _stream_ptr(stream)),
+                   "mcb_rho_static")
+        return outs[0], outs[1]
 
     def lanczos_steps(self, kmax: int = 0) -> int:
         """Steps mcb_lanczos takes for `kmax` (0: the paper's cap nc / 8, at most 1024)."""

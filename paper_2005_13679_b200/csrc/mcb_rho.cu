@@ -18,6 +18,7 @@
 //   k_rho_finish     G = sum of the partials, strided + fixed-order tree per element (deterministic).
 //   k_rho_expand     rho2 (M^4) and rho1 (M^2) from G; N = 1: rho1 = conj(C_k) C_l, rho2 = 0.
 #include <string.h>
+#include <mutex>
 #include "mcb_device.cuh"
 
 __host__ __device__ constexpr int rho_div(int a, int b) { return (a + b - 1) / b; }
@@ -287,5 +288,107 @@ extern "C" int mcb_rho(mcb_space* sp, const mcb_c128* d_C, mcb_c128* d_rho1, mcb
     case 11: return launch_rho<11>(sp, d_C, d_rho1, d_rho2, d_workspace, st);
     case 12: return launch_rho<12>(sp, d_C, d_rho1, d_rho2, d_workspace, st);
     default: return MCB_EUNSUPPORTED;
+    }
+}
+
+// =========================================================================================================
+// mcb_rho_static: the same three kernels with their scratch in a fixed array of this library (include/mcb.h)
+// =========================================================================================================
+// Who this is for: code that is handed its device buffers by a host program and has no way to ask for more -- a solver plugged
+// into an application whose own pool took the whole device at start-up (a cudaMalloc there fails, or breaks the memory budget
+// the job was given), or a propagation loop in which cudaMalloc / cudaFree are forbidden because they synchronise the whole
+// device and hold a driver lock that stalls every other stream and thread of the process.  Such a caller owns C and the two
+// result matrices but cannot produce the mcb_rho_workspace_bytes() of scratch mcb_rho wants.  Here the partial Gram matrices
+// of k_rho_gram and the reduced G of k_rho_finish live in MCB_RHO_STATIC_BYTES of device memory that belongs to the library
+// image: every device that loads libmcb.so carries it from the first use of this file's kernels until the process exits.
+//
+// In HOST code `rho_static_scratch` is only a handle of the symbol (using it as a pointer would hand the kernels a host
+// address); the device address differs per device and comes from cudaGetSymbolAddress with that device current, looked up
+// the first time this entry point runs on a device and remembered per device ordinal.
+static __device__ __align__(256) unsigned char rho_static_scratch[MCB_RHO_STATIC_BYTES];
+
+#define RHO_STATIC_MAX_DEVICES 64
+static std::mutex rho_static_mutex;
+static void* rho_static_ptr[RHO_STATIC_MAX_DEVICES];                     // device address of rho_static_scratch, by device ordinal
+
+static int rho_static_address(int device, void** out)
+{
+    std::lock_guard<std::mutex> lock(rho_static_mutex);
+    void* p = (device >= 0 && device < RHO_STATIC_MAX_DEVICES) ? rho_static_ptr[device] : NULL;
+    if (!p) {                                                            // (the caller has checked that `device` is current)
+        MCB_CUDA(cudaGetSymbolAddress(&p, rho_static_scratch));
+        if (!p || (((uintptr_t)p) & 255)) return MCB_ECUDA;
+        if (device >= 0 && device < RHO_STATIC_MAX_DEVICES) rho_static_ptr[device] = p;
+    }
+    *out = p;
+    return MCB_OK;
+}
+
+template <int M>
+static int launch_rho_static(mcb_space* sp, const mcb_c128* d_C, mcb_c128* d_rho1, mcb_c128* d_rho2, void* scratch, cudaStream_t st)
+{
+    using Cfg = RhoCfg<M>;
+    // scratch layout: G [P][P] complex | per-CTA partial matrices.  The persistent grid is cut to the number of partials the
+    // array holds (k_rho_gram strides over the tiles by gridDim.x, so any grid >= 1 is a correct one).
+    const long long g_bytes = mcb_round_up((long long)Cfg::P * Cfg::P * (long long)sizeof(double2), 256);
+    const long long per_cta = (long long)rho_parts(M) * Cfg::ROWS * Cfg::ROWS * (long long)sizeof(double);
+    const long long grid_cap = ((long long)MCB_RHO_STATIC_BYTES - g_bytes) / per_cta;
+    if (grid_cap < 1) return MCB_ESCRATCH;
+    double2* G = (double2*)scratch;
+    double* partial = (double*)((char*)scratch + g_bytes);
+    int launches = 0;
+    if (sp->N >= 2) {
+        RhoArgs a;
+        a.d = sp->dev; a.fock = sp->fock; a.C = (const double2*)d_C; a.partial = partial;
+        a.ntiles = (int)((sp->nc2 + Cfg::TM - 1) / Cfg::TM);
+        long long grid = rho_grid(sp);
+        if (grid > a.ntiles) grid = a.ntiles;
+        if (grid > grid_cap) grid = grid_cap;
+        if (!(sp->attr_set & 1u)) {
+            MCB_CUDA(cudaFuncSetAttribute(k_rho_gram<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
+            sp->attr_set |= 1u;
+        }
+        // nothing in the array has to start at zero: every CTA (warp) of this grid stores all of its block pairs, and
+        // k_rho_finish reads exactly grid * rho_parts partials -- what an earlier call left behind is never looked at
+        k_rho_gram<M><<<(int)grid, Cfg::THREADS, Cfg::SMEM, st>>>(a);
+        MCB_CHECK_LAUNCH();
+        k_rho_finish<<<Cfg::P * Cfg::P, 128, 0, st>>>(partial, (int)grid * rho_parts(M), Cfg::ROWS, Cfg::P, G);
+        MCB_CHECK_LAUNCH();
+        launches = 2;
+    }
+    const int M4 = M * M * M * M;
+    k_rho_expand<<<(M4 + 127) / 128, 128, 0, st>>>(G, (const double2*)d_C, sp->N, M, (double2*)d_rho1, (double2*)d_rho2);
+    MCB_CHECK_LAUNCH();
+    sp->last_launches = launches + 1;
+    return MCB_OK;
+}
+
+extern "C" int mcb_rho_static(mcb_space* sp, const mcb_c128* d_C, mcb_c128* d_rho1, mcb_c128* d_rho2, void* stream)
+{
+    if (!sp || !d_C || !d_rho1 || !d_rho2) return MCB_EINVAL;
+    if ((((uintptr_t)d_C) & 15) || (((uintptr_t)d_rho1) & 15) || (((uintptr_t)d_rho2) & 15)) return MCB_EINVAL;
+    if (sp->M > MCB_RHO_STATIC_MAX_M) return MCB_ESCRATCH;               // beyond: P x nc2 materialised rows, no fixed bound
+    if (sp->N >= 2 && !sp->d_fock) return MCB_ENOTREADY;
+    int device = -1;
+    MCB_CUDA(cudaGetDevice(&device));
+    if (device != sp->device) return MCB_EINVAL;                         // the space's tables live on the device it was created on
+    void* scratch = NULL;
+    const int rc = rho_static_address(device, &scratch);
+    if (rc != MCB_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    switch (sp->M) {
+    case 1: return launch_rho_static<1>(sp, d_C, d_rho1, d_rho2, scratch, st);
+    case 2: return launch_rho_static<2>(sp, d_C, d_rho1, d_rho2, scratch, st);
+    case 3: return launch_rho_static<3>(sp, d_C, d_rho1, d_rho2, scratch, st);
+    case 4: return launch_rho_static<4>(sp, d_C, d_rho1, d_rho2, scratch, st);
+    case 5: return launch_rho_static<5>(sp, d_C, d_rho1, d_rho2, scratch, st);
+    case 6: return launch_rho_static<6>(sp, d_C, d_rho1, d_rho2, scratch, st);
+    case 7: return launch_rho_static<7>(sp, d_C, d_rho1, d_rho2, scratch, st);
+    case 8: return launch_rho_static<8>(sp, d_C, d_rho1, d_rho2, scratch, st);
+    case 9: return launch_rho_static<9>(sp, d_C, d_rho1, d_rho2, scratch, st);
+    case 10: return launch_rho_static<10>(sp, d_C, d_rho1, d_rho2, scratch, st);
+    case 11: return launch_rho_static<11>(sp, d_C, d_rho1, d_rho2, scratch, st);
+    case 12: return launch_rho_static<12>(sp, d_C, d_rho1, d_rho2, scratch, st);
+    default: return MCB_ESCRATCH;
     }
 }

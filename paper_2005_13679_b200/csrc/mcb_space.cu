@@ -27,6 +27,7 @@ extern "C" const char* mcb_strerror(int status)
     case MCB_ECUDA:        return "CUDA runtime error (see mcb_last_cuda_error)";
     case MCB_ENOTREADY:    return "required structure (hashing table / jump map) not built";
     case MCB_EUNSUPPORTED: return "unsupported for this space (mode unavailable for this M or N)";
+    case MCB_ESCRATCH:     return "problem too large for the fixed scratch array of the allocation-free entry point (mcb_rho_static: M > 12)";
     default:               return "unknown status";
     }
 }
