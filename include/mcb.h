@@ -14,7 +14,8 @@
  * is computed without ever storing H.
  *
  * Conventions
- *   - every function returning int returns MCB_OK (0) or a negative MCB_E* code; nothing throws or aborts.
+ *   - every function returning int returns MCB_OK (0) or a negative MCB_E* code (mcb_lanczos alone may also return the
+ *     positive MCB_TRUNCATED, a completed run); nothing throws or aborts.
  *   - "d_" arguments are DEVICE pointers, "h_"/unprefixed array arguments are HOST pointers.
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  All device work is
  *     enqueued on it and is asynchronous unless stated otherwise.
@@ -45,6 +46,8 @@ extern "C" {
 #define MCB_ECUDA        -4   /* a CUDA runtime call failed; see mcb_last_cuda_error()                       */
 #define MCB_ENOTREADY    -5   /* a structure the call needs (hashing table, map) has not been built          */
 #define MCB_EUNSUPPORTED -6   /* mode not available for this space (see the hc_apply modes)                    */
+#define MCB_TRUNCATED     1   /* the ONE positive status: mcb_lanczos with kmax = 0 completed, but ran fewer steps than the
+                                 paper's nc / 8 because of the library's cap of 1024; results are valid       */
 #define MCB_ESCRATCH     -7   /* mcb_rho_static: the problem does not fit the library's fixed scratch array (M too large) */
 
 #define MCB_MAX_M        32   /* hashing and map kernels                                                      */
@@ -173,7 +176,9 @@ int  mcb_resolve_mode(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, int m
  * up to 16 slabs by the occupation of the last orbital: a slab's kernels start when the prefix of C it gathers from has
  * arrived and its piece of HC returns through d_HC_scratch while the next slab computes (two more streams owned by the
  * space).  Otherwise copy, apply, copy run one after the other through d_HC_scratch.  The results are those of mcb_hc_apply,
- * bit for bit. */
+ * bit for bit.  If, in the MCB_RUNS pipeline, a piece of C does not reach the device within about 4 s (a failed copy) the kernel
+ * stops waiting, finishes on what is there, and the call returns MCB_ECUDA with mcb_last_cuda_error() = cudaErrorTimeout (h_HC
+ * is then not valid). */
 int  mcb_hc_apply_host(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
                        const mcb_c128* h_C, mcb_c128* h_HC, int mode,
                        mcb_c128* d_C_scratch, mcb_c128* d_HC_scratch, void* d_workspace, void* stream);
@@ -225,6 +230,10 @@ int  mcb_rho_static(mcb_space* sp, const mcb_c128* d_C, mcb_c128* d_rho1, mcb_c1
  * beta[j] <= breakdown * max(1, |alpha[0]|) (invariant subspace); *k_done receives the number of steps taken.
  * 0 <= kmax <= 1024; kmax = 0 takes the paper's iteration cap nc / 8 (at most 1024, at least 1) --
  * mcb_lanczos_steps(sp, kmax) returns the number of steps a given kmax stands for, i.e. the length alpha and beta must have.
+ * When nc / 8 > 1024 (e.g. the paper's N = 5, M = 21: 6,641) a kmax = 0 run is cut to 1024 steps -- full re-orthogonalisation
+ * over thousands of vectors is not what the device path is sized for -- and the call returns MCB_TRUNCATED (> 0) instead of
+ * MCB_OK: alpha, beta and *k_done are valid, the caller is told that the paper's cap was not reached.
+ * T and V are packed and uploaded once per call, by its first H.C.
  * d_workspace: mcb_lanczos_workspace_bytes(sp, kmax) bytes, 256-byte aligned ((kmax + 2) vectors + scratch);
  * d_apply_workspace: as for mcb_hc_apply in `mode`.  SYNCHRONOUS (returns after the last step);
  * H must be Hermitian (T, V with the symmetries of BASELINE.json configs) for alpha to be meaningful.

@@ -18,6 +18,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmcb.so")
 
 OK, EINVAL, ERANGE, ENOMEM, ECUDA, ENOTREADY, EUNSUPPORTED, ESCRATCH = 0, -1, -2, -3, -4, -5, -6, -7
+TRUNCATED = 1          # mcb_lanczos only: completed with fewer steps than the paper's nc / 8
 FOCK_TABLE, MAP1, MAP2, MAP2C = 0, 1, 2, 3
 AUTO, MAPS, REHASH, GEMM, RUNS, SPARSE = 0, 1, 2, 3, 4, 5
 MAX_M, MAX_M_APPLY, MAX_M_TILED = 32, 32, 12
@@ -371,7 +372,8 @@ class Space:
 
     def lanczos(self, T, V, v0, kmax: int = 0, mode: int = AUTO, breakdown: float = 1e-12, stream=None):
         """(alpha [k], beta [k]) of the Lanczos tridiagonalisation of H started at the device vector v0 (k <= kmax steps;
-        kmax = 0: the paper's nc / 8).  tridiag_eigvals(alpha, beta[:-1]) gives the Ritz values."""
+        kmax = 0: the paper's nc / 8).  tridiag_eigvals(alpha, beta[:-1]) gives the Ritz values.  After the call
+        `self.lanczos_truncated` says whether a kmax = 0 run was cut below nc / 8 by the library's cap (MCB_TRUNCATED)."""
         torch = _torch()
         T = _host_c128(T, (self.M, self.M))
         V = _host_c128(V, (self.M,) * 4)
@@ -387,9 +389,12 @@ class Space:
         beta = np.zeros(steps, dtype=np.float64)
         k = ctypes.c_int(0)
         with torch.cuda.device(self.device):
-            _check(lib().mcb_lanczos(self._h, T.ctypes.data, V.ctypes.data, v0.data_ptr(), kmax, mode, breakdown,
-                                     alpha.ctypes.data, beta.ctypes.data, ctypes.byref(k), ws.data_ptr(), self._ws(mode),
-                                     _stream_ptr(stream)), "mcb_lanczos")
+            status = lib().mcb_lanczos(self._h, T.ctypes.data, V.ctypes.data, v0.data_ptr(), kmax, mode, breakdown,
+                                       alpha.ctypes.data, beta.ctypes.data, ctypes.byref(k), ws.data_ptr(), self._ws(mode),
+                                       _stream_ptr(stream))
+        self.lanczos_truncated = status == TRUNCATED
+        if status != TRUNCATED:
+            _check(status, "mcb_lanczos")
         return alpha[:k.value], beta[:k.value]
 
     def timing_enable(self, on: bool = True):

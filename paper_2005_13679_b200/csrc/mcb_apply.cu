@@ -268,16 +268,17 @@ static int launch_direct(mcb_space* sp, bool use_maps, const mcb_c128* T, const 
 {
     constexpr int P = M * (M + 1) / 2;
     // coefficients: T [M*M] complex, Vp [P*P] complex (interleaved)
-    double* h = (double*)sp->h_coef;
-    memcpy(h, T, sizeof(mcb_c128) * M * M);
-    {
+    const size_t bytes = sizeof(mcb_c128) * (size_t)(M * M + P * P);
+    if (mcb_coef_stale(sp)) {
+        double* h = (double*)sp->h_coef;
+        memcpy(h, T, sizeof(mcb_c128) * M * M);
         double* vr = h + 2 * (M * M + P * P);               // scratch behind the packed block
         double* vi = vr + P * P;
         mcb_pack_pairs(sp->N, M, T, V, false, vr, vi);
         for (int i = 0; i < P * P; ++i) { h[2 * (M * M + i)] = vr[i]; h[2 * (M * M + i) + 1] = vi[i]; }
+        { int rc = mcb_coef_upload(sp, h, bytes, st); if (rc) return rc; }
+        mcb_coef_staged(sp);
     }
-    const size_t bytes = sizeof(mcb_c128) * (size_t)(M * M + P * P);
-    { int rc = mcb_coef_upload(sp, h, bytes, st); if (rc) return rc; }
     DirectArgs a;
     a.d = sp->dev; a.fock = sp->fock;
     a.C = (const double2*)d_C; a.HC = (double2*)d_HC; a.coef = (const double2*)sp->d_coef;
@@ -381,7 +382,9 @@ static int hc_apply_host_pipelined(mcb_space* sp, const mcb_c128* T, const mcb_c
     MCB_CUDA(cudaStreamWaitEvent(st, sp->ev_b, 0));
     MCB_CUDA(cudaStreamSynchronize(st));
     *done = true;
-    if (sp->h_prog[MCB_H2D_CHUNKS] != 0) return MCB_ECUDA;              // the kernel gave up waiting for a piece of C
+    // the kernel gave up waiting for a piece of C: no CUDA call reported the failure, so record a code of our own choosing
+    // (cudaErrorTimeout) for mcb_last_cuda_error() instead of leaving a stale one there
+    if (sp->h_prog[MCB_H2D_CHUNKS] != 0) return mcb_set_cuda_error(cudaErrorTimeout);
     return MCB_OK;
 }
 

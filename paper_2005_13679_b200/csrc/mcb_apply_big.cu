@@ -271,8 +271,11 @@ int mcb_launch_big(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, const mc
         // one-body only: HC = T.C (M x M)
         const size_t bytes = sizeof(mcb_c128) * (size_t)M * M;
         if (bytes > sp->coef_bytes) return MCB_ENOMEM;
-        memcpy(sp->h_coef, T, bytes);
-        { int rc = mcb_coef_upload(sp, sp->h_coef, bytes, st); if (rc) return rc; }
+        if (mcb_coef_stale(sp)) {
+            memcpy(sp->h_coef, T, bytes);
+            { int rc = mcb_coef_upload(sp, sp->h_coef, bytes, st); if (rc) return rc; }
+            mcb_coef_staged(sp);
+        }
         { int rc = mcb_tick(sp, 0, st); if (rc) return rc; }
         k_big_onebody<<<(M + 63) / 64, 64, 0, st>>>((const double2*)sp->d_coef, (const double2*)d_C, (double2*)d_HC, M);
         MCB_CHECK_LAUNCH();
@@ -285,12 +288,15 @@ int mcb_launch_big(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, const mc
     // Vp (T folded in), interleaved complex, staged through the space's host scratch
     const size_t pp = (size_t)P * P;
     if (sizeof(double) * 4 * pp > sp->coef_bytes) return MCB_ENOMEM;
-    double* h = (double*)sp->h_coef;
-    double* vr = h + 2 * pp;
-    double* vi = vr + pp;
-    mcb_pack_pairs(sp->N, M, T, V, true, vr, vi);
-    for (size_t i = 0; i < pp; ++i) { h[2 * i] = vr[i]; h[2 * i + 1] = vi[i]; }
-    { int rc = mcb_coef_upload(sp, h, sizeof(double) * 2 * pp, st); if (rc) return rc; }
+    if (mcb_coef_stale(sp)) {                                            // (a Lanczos run stages them once: M^4 entries, 1e6 at M = 32)
+        double* h = (double*)sp->h_coef;
+        double* vr = h + 2 * pp;
+        double* vi = vr + pp;
+        mcb_pack_pairs(sp->N, M, T, V, true, vr, vi);
+        for (size_t i = 0; i < pp; ++i) { h[2 * i] = vr[i]; h[2 * i + 1] = vi[i]; }
+        { int rc = mcb_coef_upload(sp, h, sizeof(double) * 2 * pp, st); if (rc) return rc; }
+        mcb_coef_staged(sp);
+    }
     BigArgs a;
     big_args(sp, d_C, d_HC, d_ws, a);
     { int rc = mcb_tick(sp, 0, st); if (rc) return rc; }

@@ -434,20 +434,23 @@ static int launch_gemm(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
     double* vr = h + mat * Cfg::PER;
     double* vi = vr + P * P;
     if ((char*)(vi + P * P) > (char*)sp->h_coef + sp->coef_bytes) return MCB_ENOMEM;
-    mcb_pack_pairs(sp->N, M, T, V, true, vr, vi);
-    memset(h, 0, a_bytes);
-    for (int a = 0; a < P; ++a)
-        for (int c = 0; c < P; ++c) {
-            const double re = vr[a * P + c], im = vi[a * P + c];
-            if (Cfg::EMBED) {
-                h[(size_t)(2 * a) * Cfg::A_COLS + c] = re;          h[(size_t)(2 * a) * Cfg::A_COLS + P + c] = -im;
-                h[(size_t)(2 * a + 1) * Cfg::A_COLS + c] = im;      h[(size_t)(2 * a + 1) * Cfg::A_COLS + P + c] = re;
-            } else {
-                h[(size_t)a * Cfg::A_COLS + c] = re;
-                h[mat + (size_t)a * Cfg::A_COLS + c] = im;
+    if (mcb_coef_stale(sp)) {
+        mcb_pack_pairs(sp->N, M, T, V, true, vr, vi);
+        memset(h, 0, a_bytes);
+        for (int a = 0; a < P; ++a)
+            for (int c = 0; c < P; ++c) {
+                const double re = vr[a * P + c], im = vi[a * P + c];
+                if (Cfg::EMBED) {
+                    h[(size_t)(2 * a) * Cfg::A_COLS + c] = re;          h[(size_t)(2 * a) * Cfg::A_COLS + P + c] = -im;
+                    h[(size_t)(2 * a + 1) * Cfg::A_COLS + c] = im;      h[(size_t)(2 * a + 1) * Cfg::A_COLS + P + c] = re;
+                } else {
+                    h[(size_t)a * Cfg::A_COLS + c] = re;
+                    h[mat + (size_t)a * Cfg::A_COLS + c] = im;
+                }
             }
-        }
-    { int rc = mcb_coef_upload(sp, h, a_bytes, st); if (rc) return rc; }
+        { int rc = mcb_coef_upload(sp, h, a_bytes, st); if (rc) return rc; }
+        mcb_coef_staged(sp);
+    }
 
     GemmArgs g;
     g.d = sp->dev; g.fock = sp->fock;

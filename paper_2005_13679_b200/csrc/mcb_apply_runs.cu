@@ -361,10 +361,12 @@ k_hc2_runs(const RunArgs p, const __grid_constant__ RunCoef<M> coef)
                 const int need = d.nc - mcb_ldG(d.G, d.ldg, M - 2, max(d.N - (jtop + 2), 0));
                 int have;
                 // bounded: if a piece of C never arrives (a failed copy) the kernel gives up after ~4 s, raises the error
-                // word (checked by the host) and runs to completion on whatever is there instead of hanging
+                // word (checked by the host) and runs to completion on whatever is there instead of hanging.  The wait is
+                // bounded for the KERNEL, not per segment: once any warp has raised the word, nobody waits again
                 for (unsigned spins = 0;; ++spins) {
                     asm volatile("ld.acquire.sys.global.s32 %0, [%1];" : "=r"(have) : "l"(p.c_avail) : "memory");
                     if (have >= need) break;
+                    if ((spins & 63u) == 0 && *reinterpret_cast<const volatile int*>(p.tickets + 4) != 0) break;
                     if (spins > (1u << 21)) { if (lane == 0) atomicExch(p.tickets + 4, 1); break; }
                     __nanosleep(2000);
                 }
@@ -544,14 +546,17 @@ static int launch_runs(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
     RunCoef<M>& coef = *reinterpret_cast<RunCoef<M>*>(sp->runs_coef);
     double* vr = reinterpret_cast<double*>((char*)sp->runs_coef + sizeof(RunCoef<M>));
     double* vi = vr + P * P;
-    mcb_pack_pairs(sp->N, M, T, V, true, vr, vi);
-    memset(&coef, 0, sizeof(coef));
-    for (int a = 0; a < P; ++a)
-        for (int c = 0; c < P; ++c) {
-            const double re = vr[a * P + c], im = vi[a * P + c];
-            coef.b[2 * c][2 * a] = re;       coef.b[2 * c + 1][2 * a] = -im;
-            coef.b[2 * c][2 * a + 1] = im;   coef.b[2 * c + 1][2 * a + 1] = re;
-        }
+    if (mcb_coef_stale(sp)) {                                            // (held: runs_coef keeps the matrix of the run's first apply)
+        mcb_pack_pairs(sp->N, M, T, V, true, vr, vi);
+        memset(&coef, 0, sizeof(coef));
+        for (int a = 0; a < P; ++a)
+            for (int c = 0; c < P; ++c) {
+                const double re = vr[a * P + c], im = vi[a * P + c];
+                coef.b[2 * c][2 * a] = re;       coef.b[2 * c + 1][2 * a] = -im;
+                coef.b[2 * c][2 * a + 1] = im;   coef.b[2 * c + 1][2 * a + 1] = re;
+            }
+        mcb_coef_staged(sp);
+    }
 
     RunArgs a;
     a.d = sp->dev; a.fock = sp->fock;

@@ -202,14 +202,21 @@ template <int M>
 static int launch_sparse_m(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, const mcb_c128* d_C, mcb_c128* d_HC, cudaStream_t st)
 {
     int n1, n2; size_t bytes;
-    if (sparse_pack(sp, T, V, &n1, &n2, &bytes, false) < 0) return MCB_EUNSUPPORTED;
-    { int rc = mcb_coef_upload(sp, sp->h_coef, bytes, st); if (rc) return rc; }
+    if (mcb_coef_stale(sp)) {
+        if (sparse_pack(sp, T, V, &n1, &n2, &bytes, false) < 0) return MCB_EUNSUPPORTED;
+        { int rc = mcb_coef_upload(sp, sp->h_coef, bytes, st); if (rc) return rc; }
+        sp->hold_n1 = n1; sp->hold_n2 = n2; sp->hold_bytes = bytes;
+        mcb_coef_staged(sp);
+    } else { n1 = sp->hold_n1; n2 = sp->hold_n2; bytes = sp->hold_bytes; }
     SparseArgs a;
     a.d = sp->dev; a.fock = sp->fock; a.C = (const double2*)d_C; a.HC = (double2*)d_HC;
     a.coef = (const double2*)sp->d_coef; a.n1 = n1; a.n2 = n2;
     const int threads = 128;
     const size_t smem = bytes + sizeof(int) * (size_t)M * 128;          // + the CTA's occupations
-    MCB_CUDA(cudaFuncSetAttribute(k_hc_sparse<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (smem > sp->sparse_smem_set) {                                    // per space (per device); grows with the entry list only
+        MCB_CUDA(cudaFuncSetAttribute(k_hc_sparse<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        sp->sparse_smem_set = smem;
+    }
     if (sp->slabs) {
         // pipelined host apply: one launch per slab of outputs, each behind the arrival of the prefix of C it gathers from
         long long g0 = 0;

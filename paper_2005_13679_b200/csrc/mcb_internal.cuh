@@ -80,11 +80,18 @@ struct mcb_space {
     // pinned ring the packed coefficients are uploaded from (mcb_coef_upload): a pageable source would make every apply
     // synchronise with the stream; slot i is reused once the copy recorded in ev_pin[i] has completed
     void* h_pin[4]; cudaEvent_t ev_pin[4]; unsigned pin_next; int pin_state;   // pin_state: 0 not tried, 1 ready, -1 unavailable
+    // coefficient hold (mcb_lanczos: T, V and the mode are fixed for a whole run, so only its first apply packs and uploads them)
+    //   0: every apply stages its coefficients (default)   1: the next apply stages them and keeps them (-> 2)
+    //   2: what is staged (d_coef, runs_coef, the sparse list sizes below) is valid: launchers skip packing and the upload
+    int coef_hold;
+    int hold_n1, hold_n2; size_t hold_bytes;   // MCB_SPARSE: entry counts and staged bytes of the held list
     int last_launches;
     // per-space launch state (never process-wide: a process may hold spaces on several devices, used by several threads)
     void* runs_coef;           // host scratch of MCB_RUNS: coefficient matrix + packed Vp (lazily allocated)
     int runs_grid;             // persistent grid of k_hc2_runs on this space's device (0: not yet queried)
     int gemm_sms, gemm_ctas_per_sm;      // same for k_hc2_contract
+    long long maps2c_grid;     // persistent grid of k_hc_maps2c_group (0: not yet queried; its attribute is set with it)
+    size_t sparse_smem_set;    // largest dynamic shared memory size k_hc_sparse has been opted in for on this space's device
     unsigned short* d_pair_ks; // [2][P] pair index -> (k, s), device (M > MCB_MAX_M_TILED only)
     unsigned attr_set;         // bit i: cudaFuncSetAttribute done for kernel family i on this space's device
     // pipelined host apply (mcb_hc_apply_host in MCB_RUNS mode): copy stream, fork/join events, pinned progress values
@@ -110,6 +117,9 @@ int mcb_set_cuda_error(cudaError_t e);
 
 // ---- pair enumeration (k <= s), order (0,0),(0,1),..,(0,M-1),(1,1),..  (include/mcb.h) ------------------
 __host__ __device__ constexpr int mcb_pair_index(int M, int k, int s) { return k * M - k * (k - 1) / 2 + (s - k); }
+
+static inline bool mcb_coef_stale(const mcb_space* sp) { return sp->coef_hold != 2; }
+static inline void mcb_coef_staged(mcb_space* sp) { if (sp->coef_hold == 1) sp->coef_hold = 2; }
 
 // packed T, V of this call -> sp->d_coef, asynchronously on st (mcb_space.cu)
 int mcb_coef_upload(mcb_space* sp, const void* h_src, size_t bytes, cudaStream_t st);

@@ -209,8 +209,17 @@ extern "C" int mcb_lanczos(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, 
 {
     if (!sp || !T || !V || !d_v0 || !alpha || !beta || !k_done || !d_workspace) return MCB_EINVAL;
     if (kmax < 0 || kmax > LZ_MAXK) return MCB_EINVAL;
+    // kmax = 0 asks for the paper's nc / 8 steps: say so when the library's own cap cut that short
+    const bool truncated = kmax == 0 && sp->nc / 8 > LZ_MAXK;
     kmax = lz_kmax(sp, kmax);
     if (((uintptr_t)d_workspace) & 255) return MCB_EINVAL;
+    // T, V and the mode are the same for every step: resolve MCB_AUTO once (it inspects the non-zero pattern of T and V) and
+    // let the first apply stage the packed coefficients for all the others (coef_hold, mcb_internal.cuh)
+    mode = mcb_resolve_mode(sp, T, V, mode);
+    if (mode < 0) return mode;
+    // a step costs milliseconds on a large space: look at the breakdown flag after every step there, so that no apply is
+    // enqueued on a basis slot that was never written; small spaces keep the host out of the way for LZ_SYNC_EVERY steps
+    const int sync_every = sp->nc >= (1LL << 20) ? 1 : LZ_SYNC_EVERY;
     cudaStream_t st = (cudaStream_t)stream;
     const long long n = sp->nc, ld = lz_ld(sp);
     double2* basis = (double2*)d_workspace;                              // [kmax + 1][ld]
@@ -235,6 +244,7 @@ extern "C" int mcb_lanczos(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, 
     k_lz_scale<<<blocks, LZ_THREADS, 0, st>>>((const double2*)d_v0, basis, n, state);
     LZ_CUDA(cudaGetLastError());
     launches += 3;
+    sp->coef_hold = 1;
     for (int j = 0; j < kmax; ++j) {
         const int nv = j + 1;
         // (after a breakdown the remaining applies of this batch of LZ_SYNC_EVERY steps still run; their results are not used)
@@ -255,7 +265,7 @@ extern "C" int mcb_lanczos(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, 
             launches += 1;
         }
         LZ_CUDA(cudaGetLastError());
-        if ((j + 1) % LZ_SYNC_EVERY == 0 && j + 1 < kmax) {              // look at the state: stop issuing work after a breakdown
+        if ((j + 1) % sync_every == 0 && j + 1 < kmax) {              // look at the state: stop issuing work after a breakdown
             LZ_CUDA(cudaMemcpyAsync(&h->scale, &state->scale, sizeof(LzState) - offsetof(LzState, scale), cudaMemcpyDeviceToHost, st));
             LZ_CUDA(cudaStreamSynchronize(st));
             if (h->stop) break;
@@ -268,8 +278,10 @@ extern "C" int mcb_lanczos(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, 
     memcpy(alpha, h->alpha, sizeof(double) * (size_t)h->k_done);
     memcpy(beta, h->beta, sizeof(double) * (size_t)h->k_done);
     sp->last_launches = launches;
+    if (truncated) rc = MCB_TRUNCATED;
 done:
 #undef LZ_CUDA
+    sp->coef_hold = 0;
     free(h);
     return rc;
 }

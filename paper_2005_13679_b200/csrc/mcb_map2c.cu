@@ -507,13 +507,16 @@ static int launch_maps2c_group(mcb_space* sp, const M2cArgs& a, cudaStream_t st)
     const size_t smem = sizeof(double2) * P * P + 2 * sizeof(double) * (size_t)(sp->N + 3) + sizeof(int) * GROUPS * M
                         + sizeof(unsigned short) * GROUPS * P + 16;
     if (smem > 227 * 1024) return MCB_EUNSUPPORTED;
-    MCB_CUDA(cudaFuncSetAttribute(k_hc_maps2c_group<M, GS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    int per_sm = 0, sms = 0;
-    MCB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_hc_maps2c_group<M, GS>, M2C_GTHREADS, smem));
-    MCB_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, sp->device));
-    if (per_sm < 1) return MCB_EUNSUPPORTED;
+    if (sp->maps2c_grid == 0) {                                          // once per space: smem depends on (N, M) only
+        MCB_CUDA(cudaFuncSetAttribute(k_hc_maps2c_group<M, GS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int per_sm = 0, sms = 0;
+        MCB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_hc_maps2c_group<M, GS>, M2C_GTHREADS, smem));
+        MCB_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, sp->device));
+        if (per_sm < 1) return MCB_EUNSUPPORTED;
+        sp->maps2c_grid = (long long)per_sm * sms;
+    }
     long long blocks = (sp->nc + GROUPS - 1) / GROUPS;
-    if (blocks > (long long)per_sm * sms) blocks = (long long)per_sm * sms;      // persistent: Vp is staged once per block
+    if (blocks > sp->maps2c_grid) blocks = sp->maps2c_grid;              // persistent: Vp is staged once per block
     k_hc_maps2c_group<M, GS><<<(unsigned)blocks, M2C_GTHREADS, smem, st>>>(a);
     MCB_CHECK_LAUNCH();
     return MCB_OK;
@@ -524,12 +527,15 @@ int mcb_launch_maps2c(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, const
     const int P = sp->P, M = sp->M;
     const size_t pp = (size_t)P * P;
     if (sizeof(double) * 4 * pp > sp->coef_bytes) return MCB_ENOMEM;
-    double* h = (double*)sp->h_coef;
-    double* vr = h + 2 * pp;
-    double* vi = vr + pp;
-    mcb_pack_pairs(sp->N, M, T, V, true, vr, vi);                        // T folded in: no single-jump map needed
-    for (size_t i = 0; i < pp; ++i) { h[2 * i] = vr[i]; h[2 * i + 1] = vi[i]; }
-    { int rc = mcb_coef_upload(sp, h, sizeof(double) * 2 * pp, st); if (rc) return rc; }
+    if (mcb_coef_stale(sp)) {
+        double* h = (double*)sp->h_coef;
+        double* vr = h + 2 * pp;
+        double* vi = vr + pp;
+        mcb_pack_pairs(sp->N, M, T, V, true, vr, vi);                    // T folded in: no single-jump map needed
+        for (size_t i = 0; i < pp; ++i) { h[2 * i] = vr[i]; h[2 * i + 1] = vi[i]; }
+        { int rc = mcb_coef_upload(sp, h, sizeof(double) * 2 * pp, st); if (rc) return rc; }
+        mcb_coef_staged(sp);
+    }
     M2cArgs a;
     a.d = sp->dev; a.fock = sp->fock;
     a.C = (const double2*)d_C; a.HC = (double2*)d_HC; a.Vp = (const double2*)sp->d_coef;
@@ -539,6 +545,7 @@ int mcb_launch_maps2c(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, const
     { int rc = mcb_tick(sp, 0, st); if (rc) return rc; }
     int rc = MCB_EUNSUPPORTED;
     switch (M) {
+    case 1: rc = launch_maps2c_t<1>(sp, a, st); break;                   // one orbital: nc = 1, one stride of one target
     case 2: rc = launch_maps2c_t<2>(sp, a, st); break;
     case 3: rc = launch_maps2c_t<3>(sp, a, st); break;
     case 4: rc = launch_maps2c_t<4>(sp, a, st); break;

@@ -21,6 +21,7 @@ extern "C" const char* mcb_strerror(int status)
 {
     switch (status) {
     case MCB_OK:           return "ok";
+    case MCB_TRUNCATED:    return "completed, but with fewer Lanczos steps than the paper's nc / 8 (library cap 1024)";
     case MCB_EINVAL:       return "invalid argument";
     case MCB_ERANGE:       return "configuration space too large for int32 indices (or M > MCB_MAX_M)";
     case MCB_ENOMEM:       return "buffer too small or allocation failed";

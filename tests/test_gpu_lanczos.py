@@ -51,6 +51,32 @@ def test_lanczos_matches_oracle(mcb, N, M, kind):
     sp.close()
 
 
+@pytest.mark.parametrize("mode", ["GEMM", "RUNS", "REHASH", "SPARSE", "MAPS"])
+def test_lanczos_every_mode_stages_coefficients_once(mcb, mode):
+    """mcb_lanczos packs and uploads T, V in its first H.C only (every mode keeps what it staged for the rest of the run): the
+    coefficients of ALL steps must still be the oracle's, and the hold must be gone afterwards -- an apply with other matrix
+    elements right after the run uses its own."""
+    N, M = 6, 5                                                   # (the Lieb-Liniger list wants an odd M)
+    sp = mcb.Space(N, M)
+    nc = sp.nc
+    T, V, C = workloads.make_small_inputs(N, M, nc, seed=911, kind="ll" if mode == "SPARSE" else "dense")
+    sp.build_structure(mcb.FOCK_TABLE)
+    if mode == "MAPS":
+        sp.build_structure(mcb.MAP2C)
+    k = 20
+    a_ref, b_ref, _ = olz.lanczos(N, M, T, V, C, k)
+    a, b = sp.lanczos(T, V, torch.from_numpy(C).cuda(), k, mode=getattr(mcb, mode))
+    assert not sp.lanczos_truncated and len(a) == len(a_ref)
+    scale = max(1.0, np.abs(a_ref).max())
+    assert np.abs(a[:8] - a_ref[:8]).max() < 1e-9 * scale and np.abs(b[:8] - b_ref[:8]).max() < 1e-9 * scale
+    assert abs(mcb.tridiag_eigvals(a, b[:-1])[0] - olz.ritz_values(a_ref, b_ref)[0]) < 1e-9 * scale
+    T2, V2, C2 = workloads.make_small_inputs(N, M, nc, seed=912, kind="dense")
+    ref, _ = oracle.hc_apply(N, M, T2, V2, C2)
+    got = sp.hc_apply(T2, V2, torch.from_numpy(C2).cuda(), mode=getattr(mcb, mode) if mode != "SPARSE" else mcb.AUTO).cpu().numpy()
+    assert np.abs(got - ref).max() <= 1e-12 * max(np.abs(T2).max(), np.abs(V2).max()) * np.abs(C2).sum()
+    sp.close()
+
+
 def test_lanczos_lieb_liniger_ground_state_vs_ed(mcb):
     # the paper's end-to-end use (PAPER.md:323-333), shrunk: N = 5 bosons, M = 5 plane waves, g = 10
     N, M = 5, 5

@@ -77,7 +77,26 @@ def test_lanczos_paper_run_N5_M21_vs_bethe(mcb):
         sp.build_structure(mcb.FOCK_TABLE)
         v0 = workloads.random_normalised_C(sp.nc, np.random.default_rng(40 + M))
         a, b = sp.lanczos(T, V, torch.from_numpy(v0).cuda(), 0 if M == 11 else 200)
+        assert not sp.lanczos_truncated                           # nc / 8 = 375 at M = 11; an explicit kmax is never "truncated"
         e0[M] = mcb.tridiag_eigvals(a, b[:-1])[0]
         sp.close()
     assert e0[11] > e0[21] > e_bethe
     assert (e0[21] - e_bethe) < 0.6 * (e0[11] - e_bethe)         # the truncation error shrinks markedly from M = 11 to 21
+
+
+def test_lanczos_reports_when_the_paper_cap_is_cut(mcb):
+    # N = 5, M = 21 runs nc / 8 = 6,641 iterations in the paper; the library stops at 1,024 and must say so
+    N, M, g = 5, 21, 10.0
+    sp = mcb.Space(N, M)
+    assert sp.nc // 8 == 6641 and sp.lanczos_steps(0) == 1024
+    T, V, _ = workloads.lieb_liniger_TV(M, g=g)
+    sp.build_structure(mcb.FOCK_TABLE)
+    v0 = torch.from_numpy(workloads.random_normalised_C(sp.nc, np.random.default_rng(61))).cuda()
+    a200, b200 = sp.lanczos(T, V, v0, 200)
+    assert not sp.lanczos_truncated
+    a, b = sp.lanczos(T, V, v0, 0)
+    assert sp.lanczos_truncated and len(a) == 1024                # MCB_TRUNCATED: a completed, shortened run
+    assert np.abs(a[:200] - a200).max() <= 1e-9 * np.abs(a200).max()          # same run, continued
+    e200, e1024 = mcb.tridiag_eigvals(a200, b200[:-1])[0], mcb.tridiag_eigvals(a, b[:-1])[0]
+    assert bethe_E0(N, g) < e1024 <= e200 + 1e-9 * abs(e200)
+    sp.close()
