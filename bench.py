@@ -259,18 +259,76 @@ def time_mode(sp, mcb, torch, T, V, dCs, dHCs, mode, steps, warmup, barrier):
     torch.cuda.synchronize()
     barrier()
     sp.timing_enable(True)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
+    # one event per step boundary on the launching stream: the total is first-to-last, the per-step gaps give median and best
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+    evs[0].record()
     for i in range(steps):
         sp.hc_apply(T, V, dCs[i % R], out=dHCs[i % R], mode=mode)
-    e1.record()
+        evs[i + 1].record()
     torch.cuda.synchronize()
     barrier()
-    ms_total = e0.elapsed_time(e1)
+    ms_total = evs[0].elapsed_time(evs[steps])
+    time_mode.per_step_ms = [evs[i].elapsed_time(evs[i + 1]) for i in range(steps)]
     kms, la = sp.timing_read(min(steps, 512))
     sp.timing_enable(False)
     launches = int(sp.last_apply_launches())
     return ms_total, kms, launches
+
+
+def spread(ms_list):
+    """median / best / worst of per-step device times (ms)."""
+    s = sorted(ms_list)
+    return {"median_ms": s[len(s) // 2], "best_ms": s[0], "worst_ms": s[-1], "n": len(s)} if s else None
+
+
+def other_config(cfg, mcb, torch, peaks, fp64_measured, barrier, steps):
+    """A short, driver-timed line for another BASELINE.json config: device-resident H.C (MCB_AUTO), its kernels, the roofline
+    fraction of the dominant one, and the host-buffer e2e -- so that BASELINE.md's numbers for it are not the builder's alone."""
+    R = 3
+    c, T, V, Cs = workloads.make_inputs(cfg, n_vectors=R)
+    sp = mcb.Space(c.N, c.M)
+    try:
+        sp.build_structure(mcb.FOCK_TABLE)
+        mode = sp.resolve_mode(T, V, mcb.AUTO)
+        nc, nc1, nc2 = sp.nc, sp.nc_removed(1), sp.nc_removed(2)
+        tc = term_counts(c.N, c.M, nc, nc1, nc2)
+        dCs = [torch.from_numpy(C).cuda() for C in Cs]
+        dHCs = [torch.empty_like(d) for d in dCs]
+        ms_total, kms, launches = time_mode(sp, mcb, torch, T, V, dCs, dHCs, mode, steps, 3, barrier)
+        per = spread(time_mode.per_step_ms)
+        kavg = kms.mean(axis=0) if len(kms) else np.zeros(3)
+        dom = int(np.argmax(kavg)); dom_ms = float(kavg[dom])
+        out = {"workload": f"BASELINE.json configs[{cfg}] N={c.N} M={c.M} nc={nc}", "mode": MODE_NAMES[mode], "steps": steps,
+               "ms_per_step": ms_total / steps, "ms_per_step_median": per["median_ms"], "ms_per_step_best": per["best_ms"],
+               "configs_per_s": nc / (ms_total / steps * 1e-3), "gpu_launches_per_step": launches,
+               "kernel_ms": {KERNELS[mode][i]: float(kavg[i]) for i in range(len(KERNELS[mode]))}}
+        if mode == mcb.SPARSE:
+            alg = 32.0 * nc + 2.0 * c.M * nc
+            out["roofline"] = {"bound": "hbm", "kernel": KERNELS[mode][dom], "achieved": alg / (dom_ms * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
+                               "unit": "GB/s", "frac": alg / (dom_ms * 1e-3) / 1e9 / peaks["hbm_gbs"], "algorithmic_bytes_per_launch": alg}
+        else:
+            kflops = 8.0 * tc["two_body_terms_packed"] if mode in (mcb.GEMM, mcb.RUNS) else 8.0 * (tc["one_body_terms"] + tc["two_body_terms_packed"])
+            pk = fp64_measured["dmma_tflops" if mode in (mcb.GEMM, mcb.RUNS) else "dfma_tflops"]
+            out["roofline"] = {"bound": "alu", "kernel": KERNELS[mode][dom], "achieved": kflops / (dom_ms * 1e-3) / 1e12, "peak": pk,
+                               "unit": "TFLOP/s", "frac": kflops / (dom_ms * 1e-3) / 1e12 / pk, "algorithmic_flops_per_launch": kflops,
+                               "step_frac": 8.0 * (tc["one_body_terms"] + tc["two_body_terms_packed"]) / (ms_total / steps * 1e-3) / 1e12 / pk}
+        hC = [torch.from_numpy(C).pin_memory() for C in Cs]
+        hHC = [torch.empty_like(h).pin_memory() for h in hC]
+        for i in range(2):
+            sp.hc_apply_host(T, V, hC[i % R], out_host=hHC[i % R], mode=mode)
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        n_e2e = 4
+        a.record()
+        for i in range(n_e2e):
+            sp.hc_apply_host(T, V, hC[i % R], out_host=hHC[i % R], mode=mode)
+        b.record(); torch.cuda.synchronize()
+        out["e2e"] = {"ms_per_step": a.elapsed_time(b) / n_e2e, "value": nc / (a.elapsed_time(b) / n_e2e * 1e-3), "unit": UNIT,
+                      "h2d_bytes_per_step": 16 * nc + 16 * (c.M ** 2 + c.M ** 4), "d2h_bytes_per_step": 16 * nc}
+        return out
+    finally:
+        sp.close()
+        torch.cuda.empty_cache()
 
 
 def run_gpu(args):
@@ -303,7 +361,9 @@ def run_gpu(args):
     #      as GB/s of the bytes it must move against the measured HBM copy bandwidth: they are HBM-write bound by design ----
     setup = {"peak_GBps": peaks["hbm_gbs"]}
     def timed(fn, reps):
-        fn(); torch.cuda.synchronize()
+        for _ in range(3):                               # (three: rotating outputs are allocated by the first three calls)
+            fn()
+        torch.cuda.synchronize()
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a.record()
         for _ in range(reps):
@@ -312,14 +372,28 @@ def run_gpu(args):
         return a.elapsed_time(b) / reps
     def record(name, ms, nbytes):
         setup[name] = {"ms": ms, "bytes": nbytes, "GBps": nbytes / (ms * 1e-3) / 1e9, "hbm_frac": nbytes / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"]}
-    fbuf = sp.build_structure(mcb.FOCK_TABLE)
-    record("fock_table", timed(lambda: sp.build_structure(mcb.FOCK_TABLE, buf=fbuf), 5), sp.structure_bytes(mcb.FOCK_TABLE))
+    # builders write into ROTATING outputs (3 buffers, together larger than the 126 MB L2 for the big structures): rebuilding
+    # into one buffer lets L2 absorb part of the writes and the "HBM" rate is then partly an L2 rate
+    fbufs = [sp.build_structure(mcb.FOCK_TABLE) for _ in range(3)]
+    fstate = {"i": 0}
+    def build_fock():
+        fstate["i"] += 1
+        sp.build_structure(mcb.FOCK_TABLE, buf=fbufs[fstate["i"] % 3])
+    record("fock_table", timed(build_fock, 6), sp.structure_bytes(mcb.FOCK_TABLE))
+    fbuf = fbufs[0]
+    sp.build_structure(mcb.FOCK_TABLE, buf=fbuf)         # the table the applies use
+    del fbufs
+    setup["builder_outputs"] = "3 rotating output buffers per builder"
     mode = sp.resolve_mode(T, V, MODES[args.mode])       # what MCB_AUTO resolves to for these matrix elements
     if rank == 0 and not args.no_setup_rates:
+        from collections import deque
         idx_all = torch.arange(nc, dtype=torch.int32, device="cuda")
-        record("unrank_all", timed(lambda: sp.unrank(idx_all), 5), 4 * (c.M + 1) * nc)
+        alive = deque(maxlen=2)                          # the two latest outputs stay alive: each call writes a third block
+        record("unrank_all", timed(lambda: alive.append(sp.unrank(idx_all)), 6), 4 * (c.M + 1) * nc)
+        alive.clear()
         occ_all = sp.unrank(idx_all)
-        record("rank_all", timed(lambda: sp.rank(occ_all), 5), 4 * (c.M + 1) * nc)
+        record("rank_all", timed(lambda: alive.append(sp.rank(occ_all)), 6), 4 * (c.M + 1) * nc)
+        alive.clear()
         del occ_all, idx_all
         free, _ = torch.cuda.mem_get_info()
         for which, name in ((mcb.MAP1, "map1"), (mcb.MAP2, "map2")) + (((mcb.MAP2C, "map2_compact"),) if hasattr(mcb, "MAP2C") and c.N >= 2 else ()):
@@ -356,8 +430,14 @@ def run_gpu(args):
     clocks.start()
     ms_total, kms, launches = time_mode(sp, mcb, torch, T, V, dCs, dHCs, mode, args.steps, args.warmup, barrier)
     clk = clocks.stop()
+    step_spread = spread(time_mode.per_step_ms)
+    memops = sp.last_apply_memops()                       # counted by the library where the copies / memsets are issued
     ms_step = max_over_ranks(ms_total) / args.steps
     value = job.whole_job_value(nc, ms_total / args.steps)
+    # hot-cache figure (SURVEY.md 8(d) reporting rule): ONE C and ONE HC buffer, whatever of them fits stays in the 126 MB L2
+    hot_total, _, _ = time_mode(sp, mcb, torch, T, V, dCs[:1], dHCs[:1], mode, max(5, min(args.steps, 20)), 3, barrier)
+    hot = {"ms_per_step": hot_total / max(5, min(args.steps, 20)), **spread(time_mode.per_step_ms),
+           "note": "R = 1: the same C and HC every step (not the headline: inputs of the headline rotate through 3 + 3 buffers)"}
 
     # ---- end to end through the public API with HOST buffers (pinned), H2D + D2H inside the timed region ----
     hC = [torch.from_numpy(C).pin_memory() for C in Cs]
@@ -423,7 +503,9 @@ def run_gpu(args):
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": ms_step, "ms_per_step_median": step_spread["median_ms"], "ms_per_step_best": step_spread["best_ms"],
+        "ms_per_step_worst": step_spread["worst_ms"], "hot_cache": hot,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "complex128 (f64)", "data": "synthetic (seeded, workloads.py)",
         "config": dict(config_dict(c, MODE_NAMES[mode] + (f", {maps_layout}" if maps_layout else "")),
                        l2="inputs larger than L2: 3 rotating C and 3 rotating HC buffers, 16*nc bytes each",
@@ -433,9 +515,9 @@ def run_gpu(args):
         "gflop_per_step": flops_step / 1e9,
         "kernel_ms": {KERNELS[mode][i]: float(kavg[i]) for i in range(len(KERNELS[mode]))},
         "gpu_launches": launches * args.steps,
-        # what each apply enqueues besides its kernels (counted from the launchers, csrc/): one H2D copy of the packed T, V from a
-        # pinned ring (RUNS passes them as a kernel argument instead and clears its tickets / flags with one memset)
-        "gpu_memops_per_step": {"memcpy_h2d": 0 if mode == mcb.RUNS else 1, "memset": 1 if mode == mcb.RUNS else 0},
+        # what each apply enqueues besides its kernels, counted by the library at the call sites (mcb_last_apply_memops): the H2D
+        # copy of the packed T, V from a pinned ring; RUNS passes them as a kernel argument and clears its tickets with one memset
+        "gpu_memops_per_step": {"memcpy_h2d": memops[0], "memset": memops[1], "source": "mcb_last_apply_memops"},
         "roofline": roofline, "hbm_unique": hbm_unique, "setup": setup, "clocks": clk,
         "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms, "steps": e2e_steps,
                 "h2d_bytes_per_step": 16 * nc + 16 * (c.M ** 2 + c.M ** 4), "d2h_bytes_per_step": 16 * nc,
@@ -508,6 +590,18 @@ def run_gpu(args):
         except Exception as ex:
             line["lanczos"] = {"error": str(ex)}
 
+    # ---- the other BASELINE.json configs, short (rank 0, N = 1): their numbers in BASELINE.md come from here ----
+    if rank == 0 and world == 1 and not args.no_other_configs:
+        others = {}
+        for oc in (1, 2, 3, 4):
+            if oc == args.cfg:
+                continue
+            try:
+                others[f"configs[{oc}]"] = other_config(oc, mcb, torch, peaks, fp64_measured, barrier, 100 if oc == 4 else 10)
+            except Exception as ex:  # report, never hide
+                others[f"configs[{oc}]"] = {"error": str(ex)}
+        line["other_configs"] = others
+
     # ---- the oracle beside it (rank 0, N=1 only) ----
     if rank == 0 and world == 1 and not args.no_cpu:
         import oracle
@@ -571,6 +665,7 @@ def main():
     ap.add_argument("--variants", action="store_true", help="also time the other hc_apply modes (short)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-setup-rates", action="store_true", help="skip the timing of the hash / map builders")
+    ap.add_argument("--no-other-configs", action="store_true", help="skip the short lines of the other BASELINE.json configs")
     ap.add_argument("--compact-maps", action="store_true", help="--mode maps: use the paper's compact table (MCB_MAP2C) even where the dense planes fit")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--sweep", action="store_true", help="time the paper's M = 3 and N = 5 sweeps instead of the metric (one JSON line)")

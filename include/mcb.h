@@ -252,6 +252,9 @@ int  mcb_tridiag_eigvals(int n, const double* alpha, const double* beta, double*
 
 /* Number of kernels the last mcb_hc_apply / mcb_rho on this space launched (for launch accounting). */
 int  mcb_last_apply_launches(const mcb_space* sp);
+/* Copies and memsets the last mcb_hc_apply on this space enqueued beside its kernels, counted where they are issued (the
+ * upload of the packed T, V; the ticket / flag clear of MCB_RUNS).  Host ints. */
+int  mcb_last_apply_memops(const mcb_space* sp, int* memcpy_out, int* memset_out);
 
 /* ---- measurement support: device time of each kernel of hc_apply --------------------------------------------
  * mcb_timing_enable(sp, 1) clears the record and makes every following mcb_hc_apply on this space record CUDA

@@ -30,7 +30,7 @@ EXPORTS = (
     "mcb_fock_export", "mcb_map1_export", "mcb_map2_export", "mcb_map2c_export", "mcb_apply_workspace_bytes",
     "mcb_hc_apply", "mcb_hc_apply_host", "mcb_last_apply_launches", "mcb_timing_enable", "mcb_timing_read", "mcb_fp64_peak", "mcb_strerror", "mcb_last_cuda_error",
     "mcb_rho_workspace_bytes", "mcb_rho", "mcb_lanczos_workspace_bytes", "mcb_lanczos", "mcb_resolve_mode",
-    "mcb_lanczos_steps", "mcb_tridiag_eigvals", "mcb_debug_bounds", "mcb_rho_static",
+    "mcb_lanczos_steps", "mcb_tridiag_eigvals", "mcb_debug_bounds", "mcb_rho_static", "mcb_last_apply_memops",
 )
 
 _lib = None
@@ -73,6 +73,7 @@ def lib():
         L.mcb_hc_apply.argtypes = [vp, vp, vp, vp, vp, i, vp, vp]
         L.mcb_hc_apply_host.argtypes = [vp, vp, vp, vp, vp, i, vp, vp, vp, vp]
         L.mcb_last_apply_launches.argtypes = [vp]
+        L.mcb_last_apply_memops.argtypes = [vp, ctypes.POINTER(i), ctypes.POINTER(i)]
         L.mcb_timing_enable.argtypes = [vp, i]
         L.mcb_timing_read.argtypes = [vp, i, vp, vp]
         L.mcb_fp64_peak.argtypes = [i, ctypes.POINTER(ctypes.c_double), vp]
@@ -419,3 +420,9 @@ class Space:
 
     def last_apply_launches(self) -> int:
         return int(lib().mcb_last_apply_launches(self._h))
+
+    def last_apply_memops(self):
+        """(memcpy, memset) operations the last hc_apply enqueued beside its kernels, as counted by the library."""
+        a, b = ctypes.c_int(0), ctypes.c_int(0)
+        _check(lib().mcb_last_apply_memops(self._h, ctypes.byref(a), ctypes.byref(b)), "mcb_last_apply_memops")
+        return int(a.value), int(b.value)

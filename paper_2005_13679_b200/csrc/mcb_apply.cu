@@ -313,6 +313,7 @@ extern "C" int mcb_hc_apply(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
         if (c0 < h0 + len && h0 < c0 + len) return MCB_EINVAL;          // overlap
     }
     cudaStream_t st = (cudaStream_t)stream;
+    sp->n_memcpy = 0; sp->n_memset = 0;
     if (sp->M > MCB_MAX_M_TILED) {                                       // many orbitals: the generic path (mcb_apply_big.cu)
         if (mode != MCB_AUTO && mode != MCB_GEMM) return MCB_EUNSUPPORTED;
         if (sp->N >= 2) {

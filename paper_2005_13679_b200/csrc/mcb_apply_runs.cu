@@ -580,6 +580,7 @@ static int launch_runs(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
     }
     { int rc = mcb_tick(sp, 0, st); if (rc) return rc; }
     MCB_CUDA(cudaMemsetAsync(a.tickets, 0, (size_t)(mcb_round_up(a.nseg, 128) + RUNS_NTICKETS) * sizeof(int), st));
+    ++sp->n_memset;
     a.c_avail = nullptr;
     if (h_C_src) {
         // pipelined host apply: C streams in on the space's copy stream in MCB_H2D_CHUNKS pieces, each followed by a 4-byte

@@ -86,6 +86,7 @@ struct mcb_space {
     int coef_hold;
     int hold_n1, hold_n2; size_t hold_bytes;   // MCB_SPARSE: entry counts and staged bytes of the held list
     int last_launches;
+    int n_memcpy, n_memset;    // copies / memsets the last mcb_hc_apply enqueued beside its kernels (mcb_last_apply_memops)
     // per-space launch state (never process-wide: a process may hold spaces on several devices, used by several threads)
     void* runs_coef;           // host scratch of MCB_RUNS: coefficient matrix + packed Vp (lazily allocated)
     int runs_grid;             // persistent grid of k_hc2_runs on this space's device (0: not yet queried)

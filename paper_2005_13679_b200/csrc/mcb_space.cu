@@ -157,6 +157,7 @@ int mcb_coef_upload(mcb_space* sp, const void* h_src, size_t bytes, cudaStream_t
             if (ok) sp->pin_state = 1; else (void)cudaGetLastError();
         }
     }
+    ++sp->n_memcpy;
     if (sp->pin_state != 1) {                                            // large M: pageable source (the copy synchronises)
         MCB_CUDA(cudaMemcpyAsync(sp->d_coef, h_src, bytes, cudaMemcpyHostToDevice, st));
         return MCB_OK;
@@ -348,6 +349,13 @@ extern "C" int mcb_debug_bounds(const mcb_space* sp, long long* host_out)
 }
 
 extern "C" int mcb_last_apply_launches(const mcb_space* sp) { return sp ? sp->last_launches : -1; }
+
+extern "C" int mcb_last_apply_memops(const mcb_space* sp, int* memcpy_out, int* memset_out)
+{
+    if (!sp || !memcpy_out || !memset_out) return MCB_EINVAL;
+    *memcpy_out = sp->n_memcpy; *memset_out = sp->n_memset;
+    return MCB_OK;
+}
 
 // ---- per-kernel timing of hc_apply (measurement support) ----------------------------------------------------
 extern "C" int mcb_timing_enable(mcb_space* sp, int on)
