@@ -8,58 +8,86 @@
 //   * diagonal elements cost no gather at all:   T_kk n_k C_g   and   Vp[(ks)][(ks)] n_k (n_s - [k==s]) C_g
 //     (remove k, s and put them back: the target is g itself) -- an on-site interaction is entirely of this kind;
 //   * every other non-zero element (k,l) of T or ((k<=s),(q<=l)) of the packed V is one entry of a list that all
-//     threads walk together (warp-uniform control flow): the target index follows from the prefix sums S_j,
-//         index = nc - 1 - sum_{j=0}^{M-2} G[j][S_j + delta_j],   delta_j = -[j>=k] - [j>=s] + [j>=q] + [j>=l]   (mcb_device.cuh),
-//     i.e. target = g + sum_j (G[j][S_j] - G[j][S_j + delta_j]): the host packs delta_j (3 bits per j) into the entry, the
-//     thread keeps G[j][S_j] in registers and looks a table entry up only where delta_j != 0; the occupations the
-//     amplitude needs are read from a per-thread column of shared memory (run-time orbital index, no local memory).
+//     threads walk together (warp-uniform control flow).  NOTHING about an entry is decoded on the device: the host
+//     turns it into a descriptor of shared-memory row numbers, and each thread prepares, once, the few numbers of ITS
+//     configuration any entry can ask for:
+//       amplitude:  every amplitude of Eq. 12-13 is a product of at most four factors sqrt(n_j + c), c in {-1, 0, 1, 2}
+//                   (remove k, s: sqrt(n_k) sqrt(n_s - [k==s]); insert q, l into m = n - e_k - e_s: sqrt(m_q + 1)
+//                   sqrt(m_l + 1 + [q==l])) -- the thread keeps the 4 M values R[4 j + c + 1] = sqrt(n_j + c) (and a row of
+//                   ones) in its column of shared memory; a removal that is not allowed makes one factor sqrt(0) = 0;
+//       target:     index = nc - 1 - sum_{j=0}^{M-2} G[j][S_j]  (mcb_device.cuh), so the target of an entry that shifts the
+//                   prefix sum S_j by delta_j = -[j>=k] - [j>=s] + [j>=q] + [j>=l] is
+//                       g + sum_j (G[j][S_j] - G[j][S_j + delta_j]);
+//                   the j = 0 term is -delta_0 (G[0][x] = x: a constant of the entry), and for j >= 1 the thread keeps the
+//                   4 (M - 2) differences D[4 (j - 1) + code(delta)] for delta in {-2, -1, 1, 2} in its column.
+//     Per entry and thread that leaves: one descriptor (broadcast), four factor loads, the D rows with delta_j != 0, one
+//     16-byte gather of C (skipped when the amplitude is 0) and the complex multiply-add.
 // Complex FMA accumulated in registers, no atomics.  With few non-zeros the path moves from FP64-bound toward the
 // gather / HBM bound: per output 16 B of C per entry instead of P^2 products.
 #include <string.h>
 #include "mcb_device.cuh"
 
 #define MCB_SPARSE_MAX_ENTRIES 1024
+#define SPARSE_THREADS 128
 
 struct SparseArgs {
     McbDev d;
     McbFockView fock;
     const double2* C;
     double2* HC;
-    const double2* coef;       // [M] T_kk, [P] Vp diagonal, [n1 + n2] entry values, then (as int) three index words per entry
+    const double2* coef;       // [M] T_kk, [P] Vp diagonal, [nent] entry values, [nent] descriptors (int4), [nent] int (more D rows)
     int n1, n2;                // off-diagonal entries of T, of the packed V
     int g0, g1;                // outputs [g0, g1) of this launch
 };
 
+// 16-byte units of the staged coefficient block
+__host__ __device__ inline int sparse_block_units(int M, int nent) { return M + M * (M + 1) / 2 + 2 * nent + (nent + 3) / 4; }
+template <int M> struct SparseCfg {
+    static constexpr int RROWS = 4 * M + 1;                              // sqrt(n_j + c) rows + the row of ones
+    static constexpr int DROWS = M > 2 ? 4 * (M - 2) : 0;                // index differences, j = 1 .. M - 2
+    static constexpr size_t PER_CTA = (size_t)SPARSE_THREADS * (RROWS * sizeof(double) + DROWS * sizeof(int));
+};
+
 template <int M>
-__global__ void __launch_bounds__(128) k_hc_sparse(const SparseArgs p)
+__global__ void __launch_bounds__(SPARSE_THREADS) k_hc_sparse(const SparseArgs p)
 {
     constexpr int P = M * (M + 1) / 2;
-    extern __shared__ double2 sp_coef[];                    // the coefficient block, then this CTA's occupations
+    using Cfg = SparseCfg<M>;
+    extern __shared__ double2 sp_coef[];                    // the coefficient block, then the per-thread columns
     const int nent = p.n1 + p.n2;
-    const int ncoef = M + P + nent;
-    const int nwords = ncoef + (3 * nent + 3) / 4;          // + three index words per entry
-    for (int i = threadIdx.x; i < nwords; i += blockDim.x) sp_coef[i] = p.coef[i];
+    const int nunits = sparse_block_units(M, nent);
+    for (int i = threadIdx.x; i < nunits; i += SPARSE_THREADS) sp_coef[i] = p.coef[i];
     const double2* tdiag = sp_coef;
     const double2* vdiag = sp_coef + M;
     const double2* val = sp_coef + M + P;
-    const int* idx = reinterpret_cast<const int*>(sp_coef + ncoef);
-    int* occ_s = reinterpret_cast<int*>(sp_coef + nwords) + threadIdx.x;       // [M][128]: n_j of this thread at occ_s[j * 128]
+    const int4* desc = reinterpret_cast<const int4*>(sp_coef + M + P + nent);
+    const int* more = reinterpret_cast<const int*>(sp_coef + M + P + 2 * nent);
+    double* R = reinterpret_cast<double*>(sp_coef + nunits) + threadIdx.x;               // R[row * 128]
+    int* D = reinterpret_cast<int*>(reinterpret_cast<double*>(sp_coef + nunits) + Cfg::RROWS * SPARSE_THREADS) + threadIdx.x;
     const McbDev& d = p.d;
-    const int g = p.g0 + blockIdx.x * blockDim.x + threadIdx.x;
+    const int g = p.g0 + blockIdx.x * SPARSE_THREADS + threadIdx.x;
     const bool live = g < p.g1;
 
-    int S[M], G0[M];                                        // prefix sums and G[j][S_j]
     double dre = 0.0, dim = 0.0;
     {
         int n[M], run = 0;
 #pragma unroll
         for (int j = 0; j < M; ++j) {
             n[j] = live ? (int)p.fock.occ[(long long)j * p.fock.ld + g] : 0;
-            occ_s[j * 128] = n[j];
-            run += n[j]; S[j] = run;
-            G0[j] = (j + 1 < M) ? mcb_ldG(d.G, d.ldg, j, run) : 0;
+            run += n[j];
+#pragma unroll
+            for (int c = -1; c <= 2; ++c) R[(4 * j + c + 1) * SPARSE_THREADS] = __ldg(d.sq + max(n[j] + c, 0));
+            if (j >= 1 && j + 1 < M) {
+                const int g0j = mcb_ldG(d.G, d.ldg, j, run);
+#pragma unroll
+                for (int code = 0; code < 4; ++code) {
+                    const int t = run + (code < 2 ? code - 2 : code - 1);                // delta = -2, -1, +1, +2
+                    D[(4 * (j - 1) + code) * SPARSE_THREADS] = (t >= 0 && t <= d.N) ? g0j - mcb_ldG(d.G, d.ldg, j, t) : 0;
+                }
+            }
         }
-        __syncthreads();                                    // coefficient block staged (occupations are thread-private)
+        R[4 * M * SPARSE_THREADS] = 1.0;
+        __syncthreads();                                    // coefficient block staged (the columns are thread-private)
         // ---- diagonal: no gather ----
 #pragma unroll
         for (int k = 0; k < M; ++k) { dre += tdiag[k].x * n[k]; dim += tdiag[k].y * n[k]; }
@@ -77,38 +105,23 @@ __global__ void __launch_bounds__(128) k_hc_sparse(const SparseArgs p)
     const double2 cg = p.C[g];
     double2 acc = make_double2(dre * cg.x - dim * cg.y, dre * cg.y + dim * cg.x);
 
-    // ---- off-diagonal entries: one gather each.  Entry words: (k, s, q, l) bytes; then 3 bits per orbital j < M - 1
-    //      with 2 + delta_j, delta_j = -[j>=k] - [j>=s] + [j>=q] + [j>=l] the change of the prefix sum S_j: the target is
-    //      g + sum_j (G[j][S_j] - G[j][S_j + delta_j]), a look-up only where delta_j != 0 (uniform over the CTA) ----
-#pragma unroll 1
+    // ---- off-diagonal entries: descriptor = (two factor rows | two factor rows | 2 - delta_0 and the number of D rows |
+    //      five D rows of 6 bits); rows are pre-multiplied by the column stride where they fit ----
+#pragma unroll 2
     for (int e = 0; e < nent; ++e) {
-        const int w = idx[3 * e];
-        const int k = w & 255, s = (w >> 8) & 255, q = (w >> 16) & 255, l = (w >> 24) & 255;     // one-body: s = q = k (unused)
-        const bool two = e >= p.n1;
-        const int nk = occ_s[k * 128], nl = occ_s[l * 128];
-        double amp;
-        if (two) {
-            const int ns = occ_s[s * 128], nq = occ_s[q * 128];
-            const bool ok = (k == s) ? (nk >= 2) : (nk >= 1 && ns >= 1);
-            if (!ok) continue;
-            const int mq = nq - (q == k) - (q == s), ml = nl - (l == k) - (l == s);
-            const double f1 = (k == s) ? __ldg(d.sq2 + nk) : __ldg(d.sq + nk) * __ldg(d.sq + ns);
-            const double f2 = (q == l) ? __ldg(d.sq2 + mq + 2) : __ldg(d.sq + mq + 1) * __ldg(d.sq + ml + 1);
-            amp = f1 * f2;
-        } else {
-            if (nk < 1) continue;
-            amp = __ldg(d.sq + nk) * __ldg(d.sq + nl + 1);
-        }
-        int tgt = g;
-        {
-            const int wlo = idx[3 * e + 1], whi = idx[3 * e + 2];
+        const int4 ds = desc[e];
+        const double amp = (R[ds.x & 0xffff] * R[(unsigned)ds.x >> 16]) * (R[ds.y & 0xffff] * R[(unsigned)ds.y >> 16]);
+        int tgt = g + (ds.z & 7) - 2;
+        const int ng = ds.z >> 3;
 #pragma unroll
-            for (int j = 0; j + 1 < M; ++j) {
-                const int dj = (((j < 10 ? wlo >> (3 * j) : whi >> (3 * (j - 10))) & 7)) - 2;
-                if (dj != 0) tgt += G0[j] - mcb_ldG(d.G, d.ldg, j, S[j] + dj);
+        for (int t = 0; t < M - 2; ++t) {
+            if (t < ng) {
+                const int w = t < 5 ? ds.w : more[e];
+                tgt += D[((w >> (6 * (t % 5))) & 63) * SPARSE_THREADS];
             }
         }
-        const double2 z = __ldg(p.C + MCB_CHK(p.d, tgt, p.d.nc, 501));
+        double2 z = make_double2(0.0, 0.0);
+        if (amp != 0.0) z = __ldg(p.C + MCB_CHK(p.d, tgt, p.d.nc, 501));
         const double2 v = val[e];
         const double zr = amp * z.x, zi = amp * z.y;
         acc.x = fma(v.x, zr, acc.x); acc.x = fma(-v.y, zi, acc.x);
@@ -122,20 +135,39 @@ __global__ void __launch_bounds__(128) k_hc_sparse(const SparseArgs p)
 // =========================================================================================================
 // Packs T and the bosonic-symmetric part of V (mcb_pack_pairs, no folding) into the diagonal tables and the entry
 // list.  Returns the number of off-diagonal entries (n1 + n2), or -1 if the list does not fit.
-// index words of one entry: orbitals as bytes (one-body: s = q = k, never used), then 2 + delta_j in 3 bits per j
-static void sparse_words(int M, int k, int s, int q, int l, int* w)
+// Descriptor of one entry (see the kernel): one-body entries have s = q = -1.
+static void sparse_desc(int M, int k, int s, int q, int l, int* d4, int* more)
 {
     const bool two = s >= 0;
-    w[0] = k | ((two ? s : k) << 8) | ((two ? q : k) << 16) | (l << 24);
+    const int ONE = 4 * M;                                               // the row of ones
+    auto row = [&](int j, int c) { return (4 * j + c + 1) * SPARSE_THREADS; };
+    int f[4];
+    f[0] = row(k, 0);                                                    // sqrt(n_k)
+    if (two) {
+        f[1] = row(s, k == s ? -1 : 0);                                  // sqrt(n_s - [k==s])
+        f[2] = row(q, 1 - (q == k) - (q == s));                          // sqrt(m_q + 1),  m = n - e_k - e_s
+        f[3] = row(l, 1 - (l == k) - (l == s) + (q == l));               // sqrt(m_l + 1 + [q==l])
+    } else {
+        f[1] = row(l, 1);                                                // sqrt(n_l + 1)   (k != l)
+        f[2] = ONE * SPARSE_THREADS; f[3] = ONE * SPARSE_THREADS;
+    }
+    d4[0] = f[0] | (f[1] << 16);
+    d4[1] = f[2] | (f[3] << 16);
+    int ng = 0, delta0 = 0;
     unsigned long long bits = 0;
     for (int j = 0; j + 1 < M; ++j) {
         int dj = -(j >= k ? 1 : 0) + (j >= l ? 1 : 0);
         if (two) dj += -(j >= s ? 1 : 0) + (j >= q ? 1 : 0);
-        const unsigned long long f = (unsigned long long)(dj + 2);
-        if (j < 10) bits |= f << (3 * j); else bits |= f << (32 + 3 * (j - 10));
+        if (j == 0) { delta0 = dj; continue; }
+        if (dj == 0) continue;
+        const int code = dj < 0 ? dj + 2 : dj + 1;                       // -2, -1, +1, +2 -> 0, 1, 2, 3
+        const unsigned long long r = (unsigned long long)(4 * (j - 1) + code);
+        if (ng < 5) bits |= r << (6 * ng); else bits |= r << (32 + 6 * (ng - 5));
+        ++ng;
     }
-    w[1] = (int)(unsigned)(bits & 0xffffffffull);
-    w[2] = (int)(unsigned)(bits >> 32);
+    d4[2] = (2 - delta0) | (ng << 3);                                    // target = g - delta_0 + sum of the D rows
+    d4[3] = (int)(unsigned)(bits & 0xffffffffull);
+    *more = (int)(unsigned)(bits >> 32);
 }
 
 static int sparse_pack(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, int* n1_out, int* n2_out, size_t* bytes_out, bool count_only)
@@ -154,24 +186,26 @@ static int sparse_pack(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, int*
                 if (a != c && (vr[a * P + c] != 0.0 || vi[a * P + c] != 0.0)) ++n2;
     *n1_out = n1; *n2_out = n2;
     const int nent = n1 + n2;
-    const size_t bytes = sizeof(double) * 2 * (size_t)(M + P + nent) + sizeof(double) * 2 * (size_t)((3 * nent + 3) / 4);
+    const size_t bytes = sizeof(double) * 2 * (size_t)sparse_block_units(M, nent);
     *bytes_out = bytes;
     if (nent > MCB_SPARSE_MAX_ENTRIES || bytes + 2 * sizeof(double) * (size_t)P * P > sp->coef_bytes) return -1;
     if (count_only) return nent;
     double* h = (double*)sp->h_coef;
+    memset(h, 0, bytes);
     for (int k = 0; k < M; ++k) { h[2 * k] = T[k * M + k].re; h[2 * k + 1] = T[k * M + k].im; }
     for (int a = 0; a < P; ++a) {
         const bool on = sp->N >= 2;
         h[2 * (M + a)] = on ? vr[a * P + a] : 0.0; h[2 * (M + a) + 1] = on ? vi[a * P + a] : 0.0;
     }
     double* val = h + 2 * (M + P);
-    int* idx = (int*)(val + 2 * (size_t)nent);
+    int* desc = (int*)(val + 2 * (size_t)nent);
+    int* more = desc + 4 * (size_t)nent;
     int e = 0;
     for (int k = 0; k < M; ++k)
         for (int l = 0; l < M; ++l)
             if (k != l && (T[k * M + l].re != 0.0 || T[k * M + l].im != 0.0)) {
                 val[2 * e] = T[k * M + l].re; val[2 * e + 1] = T[k * M + l].im;
-                sparse_words(M, k, -1, -1, l, idx + 3 * e); ++e;
+                sparse_desc(M, k, -1, -1, l, desc + 4 * e, more + e); ++e;
             }
     if (sp->N >= 2) {
         int a = 0;
@@ -182,7 +216,7 @@ static int sparse_pack(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, int*
                     for (int l = q; l < M; ++l, ++c)
                         if (a != c && (vr[a * P + c] != 0.0 || vi[a * P + c] != 0.0)) {
                             val[2 * e] = vr[a * P + c]; val[2 * e + 1] = vi[a * P + c];
-                            sparse_words(M, k, s, q, l, idx + 3 * e); ++e;
+                            sparse_desc(M, k, s, q, l, desc + 4 * e, more + e); ++e;
                         }
             }
     }
@@ -211,8 +245,8 @@ static int launch_sparse_m(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, 
     SparseArgs a;
     a.d = sp->dev; a.fock = sp->fock; a.C = (const double2*)d_C; a.HC = (double2*)d_HC;
     a.coef = (const double2*)sp->d_coef; a.n1 = n1; a.n2 = n2;
-    const int threads = 128;
-    const size_t smem = bytes + sizeof(int) * (size_t)M * 128;          // + the CTA's occupations
+    const int threads = SPARSE_THREADS;
+    const size_t smem = bytes + SparseCfg<M>::PER_CTA;                   // + the threads' columns of factors and index differences
     if (smem > sp->sparse_smem_set) {                                    // per space (per device); grows with the entry list only
         MCB_CUDA(cudaFuncSetAttribute(k_hc_sparse<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         sp->sparse_smem_set = smem;
