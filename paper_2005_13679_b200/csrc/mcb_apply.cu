@@ -70,6 +70,23 @@ __device__ __forceinline__ void cfma(double2& acc, const double2 a, const double
     acc.y = fma(a.x, b.y, acc.y); acc.y = fma(a.y, b.x, acc.y);
 }
 
+// a map entry is read exactly once per apply: keep the stream out of L1, which the gathers of C need
+#ifndef MAPLD
+#define MAPLD 1
+#endif
+__device__ __forceinline__ int ld_map(const int* ptr)
+{
+#if MAPLD == 1
+    int v;
+    asm("ld.global.nc.L1::no_allocate.s32 %0, [%1];" : "=r"(v) : "l"(ptr));
+    return v;
+#elif MAPLD == 2
+    return __ldcs(ptr);
+#else
+    return __ldg(ptr);
+#endif
+}
+
 template <int M, bool USE_MAPS>
 __global__ void __launch_bounds__(128) k_hc_direct(DirectArgs p)
 {
@@ -133,7 +150,7 @@ __global__ void __launch_bounds__(128) k_hc_direct(DirectArgs p)
                         cfma(acc, t, make_double2(f * cg.x, f * cg.y));
                     } else {
                         int tgt;
-                        if (USE_MAPS) tgt = __ldg(p.map1 + (long long)(k * M + l) * p.ld1 + g);
+                        if (USE_MAPS) tgt = ld_map(p.map1 + (long long)(k * M + l) * p.ld1 + g);
                         else tgt = (k < l) ? g + (PM[l] - PM[k]) : g - (PP[k] - PP[l]);
                         const double2 c = __ldg(p.C + MCB_CHK(d, tgt, d.nc, 101));
                         const double f = rk[k] * rl[l];
@@ -151,7 +168,7 @@ __global__ void __launch_bounds__(128) k_hc_direct(DirectArgs p)
         int tcur[MAP_PREFETCH ? P : 1], tnext[MAP_PREFETCH ? P : 1];
         if (MAP_PREFETCH) {
 #pragma unroll
-            for (int cc = 0; cc < P; ++cc) tnext[MAP_PREFETCH ? cc : 0] = __ldg(p.map2 + (long long)cc * p.ld2 + g);
+            for (int cc = 0; cc < P; ++cc) tnext[MAP_PREFETCH ? cc : 0] = ld_map(p.map2 + (long long)cc * p.ld2 + g);
         }
         int a_run = 0;                                                   // pair counter of the rolled loops
 #pragma unroll PAIR_UNROLL
@@ -173,7 +190,7 @@ __global__ void __launch_bounds__(128) k_hc_direct(DirectArgs p)
                     if (a + 1 < P) {
                         const int* m2n = p.map2 + (long long)(a + 1) * P * p.ld2 + g;
 #pragma unroll
-                        for (int cc = 0; cc < P; ++cc) tnext[cc] = __ldg(m2n + (long long)cc * p.ld2);
+                        for (int cc = 0; cc < P; ++cc) tnext[cc] = ld_map(m2n + (long long)cc * p.ld2);
                     }
                 }
                 if (!ok) continue;
@@ -210,7 +227,7 @@ __global__ void __launch_bounds__(128) k_hc_direct(DirectArgs p)
                 for (int q = 0; q < M; ++q) {
 #pragma unroll
                     for (int l = q; l < M; ++l, ++c) {
-                        const int tgt = MAP_PREFETCH ? tcur[c] : (USE_MAPS ? __ldg(m2 + (long long)c * p.ld2) : d.nc - 1 - X[q] - Y[l]);
+                        const int tgt = MAP_PREFETCH ? tcur[c] : (USE_MAPS ? ld_map(m2 + (long long)c * p.ld2) : d.nc - 1 - X[q] - Y[l]);
                         const double2 z = __ldg(p.C + MCB_CHK(d, tgt, d.nc, 102));
                         const double f2 = (q == l) ? r2[q] : r1[q] * r1[l];
                         cfma(w, vrow[c], make_double2(f2 * z.x, f2 * z.y));
