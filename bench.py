@@ -459,7 +459,7 @@ def run_gpu(args):
     if mode == mcb.MAPS and maps_layout and maps_layout.startswith("compact"):
         KERNELS[mode] = ["k_hc_maps2c<M>"]
     if c.M > 12:
-        KERNELS[mode] = ["k_big_gather", "k_big_zgemm", "k_big_reduce"]
+        KERNELS[mode] = ["k_big_contract", "k_big_reduce"]
     dom = int(np.argmax(kavg))
     dom_ms = float(kavg[dom])
     flops_step = 8.0 * (tc["one_body_terms"] + tc["two_body_terms_packed"])

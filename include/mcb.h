@@ -54,7 +54,9 @@ extern "C" {
 #define MCB_MAX_M_APPLY  32   /* hc_apply, rho, lanczos.  Up to 12 orbitals the packed V (P x P complex, P = M(M+1)/2)
                                  lives on chip and every mode below exists; for 13 <= M <= 32 (the paper's N = 5,
                                  M <= 25 sweep) a generic path serves MCB_AUTO / MCB_GEMM and the
-                                 other modes return MCB_EUNSUPPORTED                                           */
+                                 other modes return MCB_EUNSUPPORTED.  Its workspace is 16 P nc2 bytes (not tiled over the
+                                 intermediates): 1.1 GB at N = 10, M = 16, 7.5 GB at N = 10, M = 20, 107 GB at N = 9,
+                                 M = 32 -- mcb_apply_workspace_bytes says what a space needs                    */
 #define MCB_MAX_M_RUNS    5   /* MCB_RUNS: the embedded coefficient matrix must fit in register fragments      */
 
 /* structures that live in caller-provided device memory (mcb_structure_bytes / mcb_build_structure) */

@@ -4,10 +4,10 @@
 // The packed coefficient matrix Vp (P x P complex, P = M(M+1)/2 up to 528: 4.5 MB) no longer fits on chip, M is a run-time
 // value, and the (N-2)-particle space is small when N is small (N = 5, M = 21: nc = 53,130 but nc2 = 1,771).  Same
 // factorisation through the (N-2)-particle space as MCB_GEMM (mcb_apply_gemm.cu), written for generality:
-//   k_big_gather   D[c][m] = F(m,c) C[index(m + e_q + e_l)], one thread per intermediate m, all P insertion pairs c = (q<=l)
-//                  (index = nc - 1 - X[q] - Y[l], mcb_device.cuh), materialised in the workspace (P x nc2 complex);
-//   k_big_zgemm    W'[a][m] = F(m,a) sum_c Vp[a][c] D[c][m]: a shared-memory tiled complex GEMM, Vp streamed from L2
-//                  (plain FP64 FMAs: at these shapes the whole product is a fraction of a GFLOP);
+//   k_big_contract W'[a][m] = F(m,a) sum_c Vp[a][c] F(m,c) C[index(m + e_q + e_l)] (index = nc - 1 - X[q] - Y[l],
+//                  mcb_device.cuh): the real 2P x 2P x nc2 product on mma.sync.m8n8k4.f64, 64 x 64 complex tiles, Vp streamed
+//                  from L2 and the gather of C fused into the B-tile load -- the workspace holds W' only (P x nc2 complex);
+//   k_big_gather   D[c][m] = F(m,c) C[index(m + e_q + e_l)] materialised (P x nc2 complex): the density matrices only;
 //   k_big_reduce   HC[g] = sum over the allowed removal pairs a of W'[a][index2(n^g - e_k - e_s)] -- every W' element is
 //                  read by exactly one g: no atomics.  T rides inside Vp (sum_s a+_s a_s = N), as in MCB_GEMM.
 //   k_big_gram     G[a][c] = sum_m conj(D[a][m]) D[c][m] (split over m, fixed-order finish): rho2 = G, rho1 from the number
@@ -18,9 +18,6 @@
 #include "mcb_device.cuh"
 
 #define BIG_THREADS 128
-#define BIG_BM 32                     // rows (a) per GEMM tile
-#define BIG_BN 64                     // columns (m) per GEMM tile
-#define BIG_BK 16
 #define BIG_SPLIT_MAX 64              // partial Gram matrices
 
 struct BigArgs {
@@ -80,65 +77,167 @@ __global__ void __launch_bounds__(BIG_THREADS) k_big_gather(const BigArgs p)
         }
 }
 
-// W'[a][m] = F(m,a) sum_c Vp[a][c] D[c][m].  Tile BM x BN per CTA, 128 threads: thread (ty, tx) = (tid / 16, tid % 16) owns
-// rows a = ty + 8 i (i < 4) and columns m = tx + 16 j (j < 4) of the tile: 16 complex accumulators.
-__global__ void __launch_bounds__(BIG_THREADS) k_big_zgemm(const BigArgs p, const unsigned short* __restrict__ pair_k, const unsigned short* __restrict__ pair_s)
+// ---- the contraction on the FP64 tensor path, with the gather fused into the B-tile load (no materialised D) ----------------
+// W'[a][m] = F(m,a) sum_c Vp[a][c] F(m,c) C[index(m + e_q + e_l)] as the REAL product
+//     [Re W; Im W] = [[Re Vp, -Im Vp], [Im Vp, Re Vp]] [Re D; Im D]         (2P x 2P times 2P x nc2)
+// on mma.sync.m8n8k4.f64.  CTA tile: CT_BM = 64 rows a (128 real rows: the 64 real parts, then the 64 imaginary parts) x CT_BN = 64
+// intermediates m, K walked in chunks of CT_BK = 16 insertion pairs c (32 real k: 16 real parts, then 16 imaginary parts).
+// 8 warps as 4 (32 real rows) x 2 (32 columns): 16 accumulator tiles of 8 x 8 per warp, 16 DMMAs per 8 fragment loads.
+// Once per CTA the 64 columns get their index terms X[q], Y[l] (mcb_device.cuh) and factors sqrt(m_j + 1), sqrt((m_j+1)(m_j+2))
+// in shared memory; a B element is then one gather of C and one or two multiplications.  The next chunk's global loads (Vp
+// and the gathers) are issued into registers before the DMMAs of the current chunk.
+#define CT_BM 64
+#define CT_BN 64
+#define CT_BK 16
+#define CT_THREADS 256
+#define CT_LDA (2 * CT_BK + 4)        // doubles; % 16 == 4: conflict-free A fragments
+#define CT_LDB (CT_BN + 4)            // doubles; % 16 == 4: conflict-free B fragments
+
+__device__ __forceinline__ void big_dmma884(double& c0, double& c1, const double a, const double b)
 {
-    __shared__ double2 As[BIG_BK][BIG_BM + 1];
-    __shared__ double2 Bs[BIG_BK][BIG_BN];
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+// the DMMAs of one K chunk for the first NB 8-row blocks of the warp (a branch per warp, not a predicate per DMMA: a
+// predicated-off DMMA still takes its slot in the tensor pipe)
+template <int NB>
+__device__ __forceinline__ void ct_chunk(double (&acc)[4][4][2], const double* __restrict__ xa, const double* __restrict__ xb)
+{
+#pragma unroll
+    for (int ks = 0; ks < 2 * CT_BK / 4; ++ks) {
+        double a[NB > 0 ? NB : 1], b[4];
+#pragma unroll
+        for (int i = 0; i < NB; ++i) a[i] = xa[8 * i * CT_LDA + 4 * ks];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) b[j] = xb[4 * ks * CT_LDB + 8 * j];
+#pragma unroll
+        for (int i = 0; i < NB; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) big_dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+    }
+}
+
+static size_t big_contract_smem(int M)
+{
+    return sizeof(double) * ((size_t)2 * CT_BM * CT_LDA + (size_t)2 * CT_BK * CT_LDB + (size_t)2 * M * CT_BN) + sizeof(int) * (size_t)2 * M * CT_BN;
+}
+
+__global__ void __launch_bounds__(CT_THREADS) k_big_contract(const BigArgs p, const unsigned short* __restrict__ pair_k, const unsigned short* __restrict__ pair_s)
+{
+    extern __shared__ __align__(16) double ct_smem[];
     const McbDev& d = p.d;
-    const int P = p.P;
-    const int a0 = blockIdx.y * BIG_BM, m0 = blockIdx.x * BIG_BN;
-    const int tid = threadIdx.x, ty = tid >> 4, tx = tid & 15;
-    double2 acc[4][4];
+    const int M = d.M, P = p.P;
+    double* As = ct_smem;                                                // [2 BM][LDA]
+    double* Bs = As + 2 * CT_BM * CT_LDA;                                // [2 BK][LDB]
+    double* sR1 = Bs + 2 * CT_BK * CT_LDB;                               // [M][BN] sqrt(m_j + 1)
+    double* sR2 = sR1 + M * CT_BN;                                       // [M][BN] sqrt((m_j + 1)(m_j + 2))
+    int* sX = reinterpret_cast<int*>(sR2 + M * CT_BN);                   // [M][BN]
+    int* sY = sX + M * CT_BN;                                            // [M][BN]
+    const int a0 = blockIdx.y * CT_BM, m0 = blockIdx.x * CT_BN;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int grp = lane >> 2, tig = lane & 3;
+    const int wr = warp >> 1, wc = warp & 1;
+
+    if (tid < CT_BN) {                                                   // per-column index terms and factors
+        const int m = m0 + tid;
+        int S[MCB_MAX_M], X[MCB_MAX_M], Y[MCB_MAX_M];
+        int run = 0;
+        for (int j = 0; j < M; ++j) {
+            const int nj = m < d.nc2 ? (int)p.fock.occ2[(long long)j * p.fock.ld2 + m] : 0;
+            run += nj; S[j] = run;
+            sR1[j * CT_BN + tid] = __ldg(d.sq + nj + 1);
+            sR2[j * CT_BN + tid] = __ldg(d.sq2 + nj + 2);
+        }
+        big_xy(d, S, X, Y);
+        for (int j = 0; j < M; ++j) { sX[j * CT_BN + tid] = X[j]; sY[j * CT_BN + tid] = Y[j]; }
+    }
+    __syncthreads();
+
+    // global -> register staging of one K chunk: 4 elements of Vp and 4 gathered, scaled elements of D per thread
+    const int bcol = tid & (CT_BN - 1), bk0 = tid >> 6;                  // B: column, first k of the thread (k = bk0 + 4 i)
+    const int ak = tid & (CT_BK - 1), ar0 = tid >> 4;                    // A: k within the chunk, first row (row = ar0 + 16 i)
+    const bool col_ok = m0 + bcol < d.nc2;
+    const int base = d.nc - 1;
+    double2 ra[4], rb[4];
+    auto fetch = [&](int c0) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int a = a0 + ar0 + 16 * i, c = c0 + ak;
+            ra[i] = (a < P && c < P) ? __ldg(p.Vp + (long long)a * P + c) : make_double2(0.0, 0.0);
+        }
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int c = c0 + bk0 + 4 * i;
+            double2 v = make_double2(0.0, 0.0);
+            if (c < P && col_ok) {
+                const int q = pair_k[c], l = pair_s[c];
+                const double2 z = __ldg(p.C + MCB_CHK(d, base - sX[q * CT_BN + bcol] - sY[l * CT_BN + bcol], d.nc, 203));
+                const double f = (q == l) ? sR2[q * CT_BN + bcol] : sR1[q * CT_BN + bcol] * sR1[l * CT_BN + bcol];
+                v = make_double2(f * z.x, f * z.y);
+            }
+            rb[i] = v;
+        }
+    };
+    auto stash = [&]() {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int r = ar0 + 16 * i;
+            As[r * CT_LDA + ak] = ra[i].x;              As[r * CT_LDA + CT_BK + ak] = -ra[i].y;
+            As[(CT_BM + r) * CT_LDA + ak] = ra[i].y;    As[(CT_BM + r) * CT_LDA + CT_BK + ak] = ra[i].x;
+        }
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int kk = bk0 + 4 * i;
+            Bs[kk * CT_LDB + bcol] = rb[i].x;
+            Bs[(CT_BK + kk) * CT_LDB + bcol] = rb[i].y;
+        }
+    };
+
+    double acc[4][4][2];
 #pragma unroll
     for (int i = 0; i < 4; ++i)
 #pragma unroll
-        for (int j = 0; j < 4; ++j) acc[i][j] = make_double2(0.0, 0.0);
-    for (int k0 = 0; k0 < P; k0 += BIG_BK) {
-        // A tile: Vp[a0 + r][k0 + kk], read along c (contiguous), stored transposed
-        for (int e = tid; e < BIG_BM * BIG_BK; e += BIG_THREADS) {
-            const int r = e / BIG_BK, kk = e % BIG_BK;
-            const int a = a0 + r, c = k0 + kk;
-            As[kk][r] = (a < P && c < P) ? __ldg(p.Vp + (long long)a * P + c) : make_double2(0.0, 0.0);
-        }
-        for (int e = tid; e < BIG_BK * BIG_BN; e += BIG_THREADS) {
-            const int kk = e / BIG_BN, col = e % BIG_BN;
-            const int c = k0 + kk, m = m0 + col;
-            Bs[kk][col] = (c < P && m < d.nc2) ? p.D[(long long)c * p.ld2 + m] : make_double2(0.0, 0.0);
-        }
+        for (int j = 0; j < 4; ++j) { acc[i][j][0] = 0.0; acc[i][j][1] = 0.0; }
+
+    // 8-row blocks of this warp that hold rows a < P (the last row tile is ragged: P = 136 fills 17 of its 24 blocks); the
+    // DMMAs of the empty ones are skipped, warp-uniformly
+    const int nblk = min(4, max(0, (P - (a0 + 32 * (wr & 1)) + 7) >> 3));
+    fetch(0);
+    for (int c0 = 0; c0 < P; c0 += CT_BK) {
+        stash();
         __syncthreads();
-#pragma unroll
-        for (int kk = 0; kk < BIG_BK; ++kk) {
-            double2 a[4], b[4];
-#pragma unroll
-            for (int i = 0; i < 4; ++i) a[i] = As[kk][ty + 8 * i];
-#pragma unroll
-            for (int j = 0; j < 4; ++j) b[j] = Bs[kk][tx + 16 * j];
-#pragma unroll
-            for (int i = 0; i < 4; ++i)
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    acc[i][j].x = fma(a[i].x, b[j].x, acc[i][j].x); acc[i][j].x = fma(-a[i].y, b[j].y, acc[i][j].x);
-                    acc[i][j].y = fma(a[i].x, b[j].y, acc[i][j].y); acc[i][j].y = fma(a[i].y, b[j].x, acc[i][j].y);
-                }
+        if (c0 + CT_BK < P) fetch(c0 + CT_BK);                           // in flight under the DMMAs below
+        const double* xa = As + (32 * wr + grp) * CT_LDA + tig;
+        const double* xb = Bs + tig * CT_LDB + 32 * wc + grp;
+        switch (nblk) {                                                  // warp-uniform
+        case 4: ct_chunk<4>(acc, xa, xb); break;
+        case 3: ct_chunk<3>(acc, xa, xb); break;
+        case 2: ct_chunk<2>(acc, xa, xb); break;
+        case 1: ct_chunk<1>(acc, xa, xb); break;
+        default: break;
         }
         __syncthreads();
     }
+
+    // epilogue: real row 32 wr + 8 i + grp = (part, a - a0) with part = wr >> 1; columns 32 wc + 8 j + 2 tig, + 1
+    const int part = wr >> 1;
+    double* Wd = reinterpret_cast<double*>(p.W);
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-        const int a = a0 + ty + 8 * i;
+        const int a = a0 + 32 * (wr & 1) + 8 * i + grp;
         if (a >= P) continue;
         const int k = pair_k[a], s = pair_s[a];
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-            const int m = m0 + tx + 16 * j;
-            if (m >= d.nc2) continue;
-            const int mk = (int)p.fock.occ2[(long long)k * p.fock.ld2 + m];
-            double f;
-            if (k == s) f = __ldg(d.sq2 + mk + 2);
-            else f = __ldg(d.sq + mk + 1) * __ldg(d.sq + (int)p.fock.occ2[(long long)s * p.fock.ld2 + m] + 1);
-            p.W[(long long)a * p.ld2 + m] = make_double2(f * acc[i][j].x, f * acc[i][j].y);
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const int col = 32 * wc + 8 * j + 2 * tig + e;
+                const int m = m0 + col;
+                if (m >= d.nc2) continue;
+                const double f = (k == s) ? sR2[k * CT_BN + col] : sR1[k * CT_BN + col] * sR1[s * CT_BN + col];
+                Wd[2 * ((long long)a * p.ld2 + m) + part] = f * acc[i][j][e];
+            }
         }
     }
 }
@@ -247,8 +346,8 @@ static long long big_ld2(const mcb_space* sp) { return mcb_round_up(sp->nc2 > 0 
 
 long long mcb_big_workspace_bytes(const mcb_space* sp)
 {
-    // D and W', P x ld2 complex each
-    return 2 * (long long)sp->P * big_ld2(sp) * (long long)sizeof(double2);
+    // W', P x ld2 complex (the gathered D is never materialised by the apply: k_big_contract)
+    return (long long)sp->P * big_ld2(sp) * (long long)sizeof(double2);
 }
 
 static int big_pair_tables(mcb_space* sp) { return mcb_pair_tables(sp); }
@@ -299,19 +398,22 @@ int mcb_launch_big(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, const mc
     }
     BigArgs a;
     big_args(sp, d_C, d_HC, d_ws, a);
+    a.D = nullptr; a.W = (double2*)d_ws;                                 // the workspace is W' alone
+    const size_t smem = big_contract_smem(M);
+    if (!(sp->attr_set & (1u << 9))) {
+        MCB_CUDA(cudaFuncSetAttribute(k_big_contract, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)big_contract_smem(MCB_MAX_M)));
+        sp->attr_set |= 1u << 9;
+    }
     { int rc = mcb_tick(sp, 0, st); if (rc) return rc; }
-    k_big_gather<<<(unsigned)((sp->nc2 + BIG_THREADS - 1) / BIG_THREADS), BIG_THREADS, 0, st>>>(a);
+    const dim3 grid((unsigned)((sp->nc2 + CT_BN - 1) / CT_BN), (unsigned)((P + CT_BM - 1) / CT_BM));
+    k_big_contract<<<grid, CT_THREADS, smem, st>>>(a, sp->d_pair_ks, sp->d_pair_ks + P);
     MCB_CHECK_LAUNCH();
     { int rc = mcb_tick(sp, 1, st); if (rc) return rc; }
-    const dim3 grid((unsigned)((sp->nc2 + BIG_BN - 1) / BIG_BN), (unsigned)((P + BIG_BM - 1) / BIG_BM));
-    k_big_zgemm<<<grid, BIG_THREADS, 0, st>>>(a, sp->d_pair_ks, sp->d_pair_ks + P);
-    MCB_CHECK_LAUNCH();
-    { int rc = mcb_tick(sp, 2, st); if (rc) return rc; }
     k_big_reduce<<<(unsigned)((sp->nc + BIG_THREADS - 1) / BIG_THREADS), BIG_THREADS, 0, st>>>(a);
     MCB_CHECK_LAUNCH();
-    { int rc = mcb_tick(sp, 3, st); if (rc) return rc; }
-    mcb_tick_done(sp, 3);
-    sp->last_launches = 3;
+    { int rc = mcb_tick(sp, 2, st); if (rc) return rc; }
+    mcb_tick_done(sp, 2);
+    sp->last_launches = 2;
     return MCB_OK;
 }
 

@@ -29,7 +29,8 @@ def tol(T, V, C):
     return 1e-12 * max(np.abs(T).max(), np.abs(V).max()) * np.abs(C).sum()
 
 
-@pytest.mark.parametrize("N,M,nrows", [(5, 13, 0), (2, 14, 0), (1, 20, 0), (4, 16, 0), (5, 21, 6000), (5, 25, 4000), (3, 32, 0), (6, 14, 3000)])
+@pytest.mark.parametrize("N,M,nrows", [(5, 13, 0), (2, 14, 0), (1, 20, 0), (4, 16, 0), (5, 21, 6000), (5, 25, 4000), (3, 32, 0), (6, 14, 3000),
+                                          (8, 14, 2000)])            # nc2 = 27,132: 424 column tiles with a ragged tail, 2 row tiles
 def test_hc_apply_many_orbitals(mcb, N, M, nrows):
     sp = mcb.Space(N, M)
     nc = sp.nc
@@ -44,7 +45,7 @@ def test_hc_apply_many_orbitals(mcb, N, M, nrows):
         got = got[rows]
     err = np.abs(got - ref).max()
     assert err <= tol(T, V, C), (err, tol(T, V, C))
-    assert sp.resolve_mode(T, V) == mcb.GEMM and sp.last_apply_launches() == (3 if N >= 2 else 1)
+    assert sp.resolve_mode(T, V) == mcb.GEMM and sp.last_apply_launches() == (2 if N >= 2 else 1)
     # host path and a second call through the same workspace
     again = sp.hc_apply_host(T, V, C).numpy()
     assert np.array_equal(again if rows is None else again[rows], got)
