@@ -81,14 +81,16 @@ __global__ void __launch_bounds__(BIG_THREADS) k_big_gather(const BigArgs p)
 // W'[a][m] = F(m,a) sum_c Vp[a][c] F(m,c) C[index(m + e_q + e_l)] as the REAL product
 //     [Re W; Im W] = [[Re Vp, -Im Vp], [Im Vp, Re Vp]] [Re D; Im D]         (2P x 2P times 2P x nc2)
 // on mma.sync.m8n8k4.f64.  CTA tile: CT_BM = 64 rows a (128 real rows: the 64 real parts, then the 64 imaginary parts) x CT_BN = 64
-// intermediates m, K walked in chunks of CT_BK = 16 insertion pairs c (32 real k: 16 real parts, then 16 imaginary parts).
+// intermediates m, K walked in chunks of CT_BK = 8 insertion pairs c (16 real k: 8 real parts, then 8 imaginary parts), the
+// tiles of two chunks in shared memory (one barrier per chunk: a warp stores the next chunk as soon as ITS DMMAs are done).
 // 8 warps as 4 (32 real rows) x 2 (32 columns): 16 accumulator tiles of 8 x 8 per warp, 16 DMMAs per 8 fragment loads.
 // Once per CTA the 64 columns get their index terms X[q], Y[l] (mcb_device.cuh) and factors sqrt(m_j + 1), sqrt((m_j+1)(m_j+2))
 // in shared memory; a B element is then one gather of C and one or two multiplications.  The next chunk's global loads (Vp
 // and the gathers) are issued into registers before the DMMAs of the current chunk.
 #define CT_BM 64
 #define CT_BN 64
-#define CT_BK 16
+#define CT_BK 8
+#define CT_PER (CT_BM * CT_BK / CT_THREADS)   // elements of an A tile (and of a B tile) per thread and chunk
 #define CT_THREADS 256
 #define CT_LDA (2 * CT_BK + 4)        // doubles; % 16 == 4: conflict-free A fragments
 #define CT_LDB (CT_BN + 4)            // doubles; % 16 == 4: conflict-free B fragments
@@ -120,7 +122,7 @@ __device__ __forceinline__ void ct_chunk(double (&acc)[4][4][2], const double* _
 
 static size_t big_contract_smem(int M)
 {
-    return sizeof(double) * ((size_t)2 * CT_BM * CT_LDA + (size_t)2 * CT_BK * CT_LDB + (size_t)2 * M * CT_BN) + sizeof(int) * (size_t)2 * M * CT_BN;
+    return sizeof(double) * (2 * ((size_t)2 * CT_BM * CT_LDA + (size_t)2 * CT_BK * CT_LDB) + (size_t)2 * M * CT_BN) + sizeof(int) * (size_t)2 * M * CT_BN;
 }
 
 __global__ void __launch_bounds__(CT_THREADS) k_big_contract(const BigArgs p, const unsigned short* __restrict__ pair_k, const unsigned short* __restrict__ pair_s)
@@ -128,9 +130,8 @@ __global__ void __launch_bounds__(CT_THREADS) k_big_contract(const BigArgs p, co
     extern __shared__ __align__(16) double ct_smem[];
     const McbDev& d = p.d;
     const int M = d.M, P = p.P;
-    double* As = ct_smem;                                                // [2 BM][LDA]
-    double* Bs = As + 2 * CT_BM * CT_LDA;                                // [2 BK][LDB]
-    double* sR1 = Bs + 2 * CT_BK * CT_LDB;                               // [M][BN] sqrt(m_j + 1)
+    constexpr int STAGE = 2 * CT_BM * CT_LDA + 2 * CT_BK * CT_LDB;       // doubles per stage: A [2 BM][LDA], then B [2 BK][LDB]
+    double* sR1 = ct_smem + 2 * STAGE;                                   // [M][BN] sqrt(m_j + 1)
     double* sR2 = sR1 + M * CT_BN;                                       // [M][BN] sqrt((m_j + 1)(m_j + 2))
     int* sX = reinterpret_cast<int*>(sR2 + M * CT_BN);                   // [M][BN]
     int* sY = sX + M * CT_BN;                                            // [M][BN]
@@ -156,41 +157,44 @@ __global__ void __launch_bounds__(CT_THREADS) k_big_contract(const BigArgs p, co
 
     // global -> register staging of one K chunk: 4 elements of Vp and 4 gathered, scaled elements of D per thread
     const int bcol = tid & (CT_BN - 1), bk0 = tid >> 6;                  // B: column, first k of the thread (k = bk0 + 4 i)
-    const int ak = tid & (CT_BK - 1), ar0 = tid >> 4;                    // A: k within the chunk, first row (row = ar0 + 16 i)
+    const int ak = tid & (CT_BK - 1), ar0 = tid / CT_BK;                 // A: k within the chunk, first row (row = ar0 + AR i)
+    constexpr int AR = CT_THREADS / CT_BK;
     const bool col_ok = m0 + bcol < d.nc2;
     const int base = d.nc - 1;
-    double2 ra[4], rb[4];
-    auto fetch = [&](int c0) {
+    double2 ra[CT_PER], rb[CT_PER];
+    double rf[CT_PER];                                                   // F(m,c): multiplied in at the stash, AFTER the DMMAs -- the
+    auto fetch = [&](int c0) {                                           // gathered value must not be touched while it is in flight
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            const int a = a0 + ar0 + 16 * i, c = c0 + ak;
+        for (int i = 0; i < CT_PER; ++i) {
+            const int a = a0 + ar0 + AR * i, c = c0 + ak;
             ra[i] = (a < P && c < P) ? __ldg(p.Vp + (long long)a * P + c) : make_double2(0.0, 0.0);
         }
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
+        for (int i = 0; i < CT_PER; ++i) {
             const int c = c0 + bk0 + 4 * i;
-            double2 v = make_double2(0.0, 0.0);
+            rb[i] = make_double2(0.0, 0.0);
+            rf[i] = 0.0;
             if (c < P && col_ok) {
                 const int q = pair_k[c], l = pair_s[c];
-                const double2 z = __ldg(p.C + MCB_CHK(d, base - sX[q * CT_BN + bcol] - sY[l * CT_BN + bcol], d.nc, 203));
-                const double f = (q == l) ? sR2[q * CT_BN + bcol] : sR1[q * CT_BN + bcol] * sR1[l * CT_BN + bcol];
-                v = make_double2(f * z.x, f * z.y);
+                rb[i] = __ldg(p.C + MCB_CHK(d, base - sX[q * CT_BN + bcol] - sY[l * CT_BN + bcol], d.nc, 203));
+                rf[i] = (q == l) ? sR2[q * CT_BN + bcol] : sR1[q * CT_BN + bcol] * sR1[l * CT_BN + bcol];
             }
-            rb[i] = v;
         }
     };
-    auto stash = [&]() {
+    auto stash = [&](int stage) {
+        double* As = ct_smem + stage * STAGE;
+        double* Bs = As + 2 * CT_BM * CT_LDA;
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            const int r = ar0 + 16 * i;
+        for (int i = 0; i < CT_PER; ++i) {
+            const int r = ar0 + AR * i;
             As[r * CT_LDA + ak] = ra[i].x;              As[r * CT_LDA + CT_BK + ak] = -ra[i].y;
             As[(CT_BM + r) * CT_LDA + ak] = ra[i].y;    As[(CT_BM + r) * CT_LDA + CT_BK + ak] = ra[i].x;
         }
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
+        for (int i = 0; i < CT_PER; ++i) {
             const int kk = bk0 + 4 * i;
-            Bs[kk * CT_LDB + bcol] = rb[i].x;
-            Bs[(CT_BK + kk) * CT_LDB + bcol] = rb[i].y;
+            Bs[kk * CT_LDB + bcol] = rf[i] * rb[i].x;
+            Bs[(CT_BK + kk) * CT_LDB + bcol] = rf[i] * rb[i].y;
         }
     };
 
@@ -204,12 +208,14 @@ __global__ void __launch_bounds__(CT_THREADS) k_big_contract(const BigArgs p, co
     // DMMAs of the empty ones are skipped, warp-uniformly
     const int nblk = min(4, max(0, (P - (a0 + 32 * (wr & 1)) + 7) >> 3));
     fetch(0);
-    for (int c0 = 0; c0 < P; c0 += CT_BK) {
-        stash();
-        __syncthreads();
-        if (c0 + CT_BK < P) fetch(c0 + CT_BK);                           // in flight under the DMMAs below
-        const double* xa = As + (32 * wr + grp) * CT_LDA + tig;
-        const double* xb = Bs + tig * CT_LDB + 32 * wc + grp;
+    stash(0);
+    __syncthreads();
+    int stage = 0;
+    for (int c0 = 0; c0 < P; c0 += CT_BK, stage ^= 1) {
+        const bool more = c0 + CT_BK < P;
+        if (more) fetch(c0 + CT_BK);                                     // in flight under the DMMAs below
+        const double* xa = ct_smem + stage * STAGE + (32 * wr + grp) * CT_LDA + tig;
+        const double* xb = ct_smem + stage * STAGE + 2 * CT_BM * CT_LDA + tig * CT_LDB + 32 * wc + grp;
         switch (nblk) {                                                  // warp-uniform
         case 4: ct_chunk<4>(acc, xa, xb); break;
         case 3: ct_chunk<3>(acc, xa, xb); break;
@@ -217,6 +223,8 @@ __global__ void __launch_bounds__(CT_THREADS) k_big_contract(const BigArgs p, co
         case 1: ct_chunk<1>(acc, xa, xb); break;
         default: break;
         }
+        // the other stage was last read in the previous iteration, before its closing barrier: free to overwrite now
+        if (more) stash(stage ^ 1);
         __syncthreads();
     }
 
