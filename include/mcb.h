@@ -53,8 +53,9 @@ extern "C" {
 #define MCB_MAX_M        32   /* hashing and map kernels                                                      */
 #define MCB_MAX_M_APPLY  32   /* hc_apply, rho, lanczos.  Up to 12 orbitals the packed V (P x P complex, P = M(M+1)/2)
                                  lives on chip and every mode below exists; for 13 <= M <= 32 (the paper's N = 5,
-                                 M <= 25 sweep) a generic path serves MCB_AUTO / MCB_GEMM and the
-                                 other modes return MCB_EUNSUPPORTED.  Its workspace is 16 P nc2 bytes (not tiled over the
+                                 M <= 25 sweep) a generic path serves MCB_AUTO / MCB_GEMM, MCB_SPARSE
+                                 has a run-time-M kernel (lattices of more than 12 sites), and the other modes return
+                                 MCB_EUNSUPPORTED.  Its workspace is 16 P nc2 bytes (not tiled over the
                                  intermediates): 1.1 GB at N = 10, M = 16, 7.5 GB at N = 10, M = 20, 107 GB at N = 9,
                                  M = 32 -- mcb_apply_workspace_bytes says what a space needs                    */
 #define MCB_MAX_M_RUNS    5   /* MCB_RUNS: the embedded coefficient matrix must fit in register fragments      */
@@ -160,7 +161,7 @@ long long mcb_apply_workspace_bytes(const mcb_space* sp, int mode);
  *      packs exactly that part.  T, V are read before the call returns.
  *   d_C, d_HC: device, nc complex each, 16-byte aligned, must not overlap.
  *   d_workspace: device, mcb_apply_workspace_bytes(sp, mode) bytes, 256-byte aligned (may be NULL if 0).
- * Asynchronous on `stream`.  M must be <= MCB_MAX_M_APPLY (modes other than MCB_AUTO / MCB_GEMM: M <= 12). */
+ * Asynchronous on `stream`.  M must be <= MCB_MAX_M_APPLY (modes other than MCB_AUTO / MCB_GEMM / MCB_SPARSE: M <= 12). */
 int  mcb_hc_apply(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
                   const mcb_c128* d_C, mcb_c128* d_HC, int mode, void* d_workspace, void* stream);
 

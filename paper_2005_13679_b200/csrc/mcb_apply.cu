@@ -270,8 +270,10 @@ extern "C" long long mcb_apply_workspace_bytes(const mcb_space* sp, int mode)
     if (!sp) return MCB_EINVAL;
     if (sp->M > MCB_MAX_M_APPLY) return MCB_EUNSUPPORTED;
     if (mode < MCB_AUTO || mode > MCB_SPARSE) return MCB_EINVAL;
-    if (sp->M > MCB_MAX_M_TILED)                                         // many orbitals: the generic path (mcb_apply_big.cu)
+    if (sp->M > MCB_MAX_M_TILED) {                                       // many orbitals: the generic path (mcb_apply_big.cu), or SPARSE
+        if (mode == MCB_SPARSE) return 0;
         return (mode == MCB_AUTO || mode == MCB_GEMM) ? (sp->N >= 2 ? mcb_big_workspace_bytes(sp) : 0) : (long long)MCB_EUNSUPPORTED;
+    }
     if (mode == MCB_SPARSE) return 0;
     mode = resolve_mode(sp, mode);
     if (mode == MCB_RUNS) return mcb_runs_supported(sp) ? mcb_runs_workspace_bytes(sp) : (long long)MCB_EUNSUPPORTED;
@@ -331,7 +333,11 @@ extern "C" int mcb_hc_apply(mcb_space* sp, const mcb_c128* T, const mcb_c128* V,
     }
     cudaStream_t st = (cudaStream_t)stream;
     sp->n_memcpy = 0; sp->n_memset = 0;
-    if (sp->M > MCB_MAX_M_TILED) {                                       // many orbitals: the generic path (mcb_apply_big.cu)
+    if (sp->M > MCB_MAX_M_TILED) {                                       // many orbitals: the generic path (mcb_apply_big.cu), or SPARSE
+        if (mode == MCB_SPARSE || (mode == MCB_AUTO && sp->d_fock && mcb_sparse_preferred(sp, T, V))) {
+            if (!sp->d_fock) return MCB_ENOTREADY;
+            return mcb_launch_sparse(sp, T, V, d_C, d_HC, st);
+        }
         if (mode != MCB_AUTO && mode != MCB_GEMM) return MCB_EUNSUPPORTED;
         if (sp->N >= 2) {
             if (!sp->d_fock) return MCB_ENOTREADY;
@@ -367,7 +373,10 @@ extern "C" int mcb_resolve_mode(mcb_space* sp, const mcb_c128* T, const mcb_c128
     if (!sp || !T || !V) return MCB_EINVAL;
     if (mode < MCB_AUTO || mode > MCB_SPARSE) return MCB_EINVAL;
     if (sp->M > MCB_MAX_M_APPLY) return MCB_EUNSUPPORTED;
-    if (sp->M > MCB_MAX_M_TILED) return (mode == MCB_AUTO || mode == MCB_GEMM) ? MCB_GEMM : MCB_EUNSUPPORTED;
+    if (sp->M > MCB_MAX_M_TILED) {
+        if (mode == MCB_SPARSE || (mode == MCB_AUTO && sp->d_fock && mcb_sparse_preferred(sp, T, V))) return MCB_SPARSE;
+        return (mode == MCB_AUTO || mode == MCB_GEMM) ? MCB_GEMM : MCB_EUNSUPPORTED;
+    }
     if (mode == MCB_SPARSE || (mode == MCB_AUTO && mcb_sparse_preferred(sp, T, V))) return MCB_SPARSE;
     return resolve_mode(sp, mode);
 }

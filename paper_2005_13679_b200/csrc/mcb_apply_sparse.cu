@@ -130,17 +130,102 @@ __global__ void __launch_bounds__(SPARSE_THREADS) k_hc_sparse(const SparseArgs p
     p.HC[g] = acc;
 }
 
+// ---- many orbitals (12 < M <= 32; a Bose-Hubbard lattice is naturally larger than 12 sites): the same kernel with
+// M a run-time value.  64 threads per CTA (the columns of a thread take 4 M + 1 doubles and 5 M - 8 ints: 113 KB per CTA at
+// M = 32), the occupations kept in the thread's column for the diagonal sums, and the D rows of an entry listed as bytes
+// (up to M - 2 = 30 of them, 32 bytes per entry) instead of 6-bit fields.
+#define SPARSE_RT_THREADS 64
+__host__ __device__ inline int sparse_rt_block_units(int M, int nent) { return M + M * (M + 1) / 2 + 4 * nent; }
+static size_t sparse_rt_per_cta(int M)
+{
+    return (size_t)SPARSE_RT_THREADS * ((4 * M + 1) * sizeof(double) + (4 * (M - 2) + M) * sizeof(int));
+}
+
+__global__ void __launch_bounds__(SPARSE_RT_THREADS) k_hc_sparse_rt(const SparseArgs p)
+{
+    const McbDev& d = p.d;
+    const int M = d.M, P = M * (M + 1) / 2;
+    extern __shared__ double2 sp_coef[];
+    const int nent = p.n1 + p.n2;
+    const int nunits = sparse_rt_block_units(M, nent);
+    for (int i = threadIdx.x; i < nunits; i += SPARSE_RT_THREADS) sp_coef[i] = p.coef[i];
+    const double2* tdiag = sp_coef;
+    const double2* vdiag = sp_coef + M;
+    const double2* val = sp_coef + M + P;
+    const int4* desc = reinterpret_cast<const int4*>(sp_coef + M + P + nent);
+    const unsigned char* rows = reinterpret_cast<const unsigned char*>(sp_coef + M + P + 2 * nent);      // [nent][32]
+    double* R = reinterpret_cast<double*>(sp_coef + nunits) + threadIdx.x;                               // R[row * 64]
+    int* D = reinterpret_cast<int*>(reinterpret_cast<double*>(sp_coef + nunits) + (4 * M + 1) * SPARSE_RT_THREADS) + threadIdx.x;
+    int* Nn = D + 4 * (M - 2) * SPARSE_RT_THREADS;                                                      // Nn[j * 64]
+    const int g = p.g0 + blockIdx.x * SPARSE_RT_THREADS + threadIdx.x;
+    const bool live = g < p.g1;
+    {
+        int run = 0;
+        for (int j = 0; j < M; ++j) {
+            const int nj = live ? (int)p.fock.occ[(long long)j * p.fock.ld + g] : 0;
+            Nn[j * SPARSE_RT_THREADS] = nj;
+            run += nj;
+#pragma unroll
+            for (int c = -1; c <= 2; ++c) R[(4 * j + c + 1) * SPARSE_RT_THREADS] = __ldg(d.sq + max(nj + c, 0));
+            if (j >= 1 && j + 1 < M) {
+                const int g0j = mcb_ldG(d.G, d.ldg, j, run);
+#pragma unroll
+                for (int code = 0; code < 4; ++code) {
+                    const int t = run + (code < 2 ? code - 2 : code - 1);
+                    D[(4 * (j - 1) + code) * SPARSE_RT_THREADS] = (t >= 0 && t <= d.N) ? g0j - mcb_ldG(d.G, d.ldg, j, t) : 0;
+                }
+            }
+        }
+        R[4 * M * SPARSE_RT_THREADS] = 1.0;
+    }
+    __syncthreads();
+    if (!live) return;
+    double dre = 0.0, dim = 0.0;
+    {
+        int a = 0;
+        for (int k = 0; k < M; ++k) {
+            const int nk = Nn[k * SPARSE_RT_THREADS];
+            dre += tdiag[k].x * nk; dim += tdiag[k].y * nk;
+            if (nk == 0) { a += M - k; continue; }                       // every pair (k, s) of an empty orbital k contributes 0
+            for (int s = k; s < M; ++s, ++a) {
+                const double f = (double)(nk * (Nn[s * SPARSE_RT_THREADS] - (k == s ? 1 : 0)));
+                dre += vdiag[a].x * f; dim += vdiag[a].y * f;
+            }
+        }
+    }
+    const double2 cg = p.C[g];
+    double2 acc = make_double2(dre * cg.x - dim * cg.y, dre * cg.y + dim * cg.x);
+#pragma unroll 1
+    for (int e = 0; e < nent; ++e) {
+        const int4 ds = desc[e];
+        const double amp = (R[ds.x & 0xffff] * R[(unsigned)ds.x >> 16]) * (R[ds.y & 0xffff] * R[(unsigned)ds.y >> 16]);
+        if (amp == 0.0) continue;
+        int tgt = g + (ds.z & 7) - 2;
+        const int ng = ds.z >> 3;
+        const unsigned char* rw = rows + 32 * e;
+        for (int t = 0; t < ng; ++t) tgt += D[(int)rw[t] * SPARSE_RT_THREADS];
+        const double2 z = __ldg(p.C + MCB_CHK(p.d, tgt, p.d.nc, 502));
+        const double2 v = val[e];
+        const double zr = amp * z.x, zi = amp * z.y;
+        acc.x = fma(v.x, zr, acc.x); acc.x = fma(-v.y, zi, acc.x);
+        acc.y = fma(v.x, zi, acc.y); acc.y = fma(v.y, zr, acc.y);
+    }
+    p.HC[g] = acc;
+}
+
 // =========================================================================================================
 // host
 // =========================================================================================================
 // Packs T and the bosonic-symmetric part of V (mcb_pack_pairs, no folding) into the diagonal tables and the entry
 // list.  Returns the number of off-diagonal entries (n1 + n2), or -1 if the list does not fit.
 // Descriptor of one entry (see the kernel): one-body entries have s = q = -1.
-static void sparse_desc(int M, int k, int s, int q, int l, int* d4, int* more)
+// (M > MCB_MAX_M_TILED: column stride of k_hc_sparse_rt, and the D rows as bytes in rows32[32] instead of the 6-bit fields)
+static void sparse_desc(int M, int k, int s, int q, int l, int* d4, int* more, unsigned char* rows32)
 {
     const bool two = s >= 0;
     const int ONE = 4 * M;                                               // the row of ones
-    auto row = [&](int j, int c) { return (4 * j + c + 1) * SPARSE_THREADS; };
+    const int STRIDE = rows32 ? SPARSE_RT_THREADS : SPARSE_THREADS;
+    auto row = [&](int j, int c) { return (4 * j + c + 1) * STRIDE; };
     int f[4];
     f[0] = row(k, 0);                                                    // sqrt(n_k)
     if (two) {
@@ -149,7 +234,7 @@ static void sparse_desc(int M, int k, int s, int q, int l, int* d4, int* more)
         f[3] = row(l, 1 - (l == k) - (l == s) + (q == l));               // sqrt(m_l + 1 + [q==l])
     } else {
         f[1] = row(l, 1);                                                // sqrt(n_l + 1)   (k != l)
-        f[2] = ONE * SPARSE_THREADS; f[3] = ONE * SPARSE_THREADS;
+        f[2] = ONE * STRIDE; f[3] = ONE * STRIDE;
     }
     d4[0] = f[0] | (f[1] << 16);
     d4[1] = f[2] | (f[3] << 16);
@@ -162,12 +247,13 @@ static void sparse_desc(int M, int k, int s, int q, int l, int* d4, int* more)
         if (dj == 0) continue;
         const int code = dj < 0 ? dj + 2 : dj + 1;                       // -2, -1, +1, +2 -> 0, 1, 2, 3
         const unsigned long long r = (unsigned long long)(4 * (j - 1) + code);
-        if (ng < 5) bits |= r << (6 * ng); else bits |= r << (32 + 6 * (ng - 5));
+        if (rows32) rows32[ng] = (unsigned char)r;
+        else if (ng < 5) bits |= r << (6 * ng); else bits |= r << (32 + 6 * (ng - 5));
         ++ng;
     }
     d4[2] = (2 - delta0) | (ng << 3);                                    // target = g - delta_0 + sum of the D rows
     d4[3] = (int)(unsigned)(bits & 0xffffffffull);
-    *more = (int)(unsigned)(bits >> 32);
+    if (more) *more = (int)(unsigned)(bits >> 32);
 }
 
 static int sparse_pack(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, int* n1_out, int* n2_out, size_t* bytes_out, bool count_only)
@@ -186,7 +272,8 @@ static int sparse_pack(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, int*
                 if (a != c && (vr[a * P + c] != 0.0 || vi[a * P + c] != 0.0)) ++n2;
     *n1_out = n1; *n2_out = n2;
     const int nent = n1 + n2;
-    const size_t bytes = sizeof(double) * 2 * (size_t)sparse_block_units(M, nent);
+    const bool rt = M > MCB_MAX_M_TILED;
+    const size_t bytes = sizeof(double) * 2 * (size_t)(rt ? sparse_rt_block_units(M, nent) : sparse_block_units(M, nent));
     *bytes_out = bytes;
     if (nent > MCB_SPARSE_MAX_ENTRIES || bytes + 2 * sizeof(double) * (size_t)P * P > sp->coef_bytes) return -1;
     if (count_only) return nent;
@@ -200,12 +287,15 @@ static int sparse_pack(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, int*
     double* val = h + 2 * (M + P);
     int* desc = (int*)(val + 2 * (size_t)nent);
     int* more = desc + 4 * (size_t)nent;
+    unsigned char* rows32 = (unsigned char*)more;                        // run-time-M layout: 32 bytes per entry behind the descriptors
     int e = 0;
     for (int k = 0; k < M; ++k)
         for (int l = 0; l < M; ++l)
             if (k != l && (T[k * M + l].re != 0.0 || T[k * M + l].im != 0.0)) {
                 val[2 * e] = T[k * M + l].re; val[2 * e + 1] = T[k * M + l].im;
-                sparse_desc(M, k, -1, -1, l, desc + 4 * e, more + e); ++e;
+                if (rt) sparse_desc(M, k, -1, -1, l, desc + 4 * e, nullptr, rows32 + 32 * (size_t)e);
+                else sparse_desc(M, k, -1, -1, l, desc + 4 * e, more + e, nullptr);
+                ++e;
             }
     if (sp->N >= 2) {
         int a = 0;
@@ -216,7 +306,9 @@ static int sparse_pack(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, int*
                     for (int l = q; l < M; ++l, ++c)
                         if (a != c && (vr[a * P + c] != 0.0 || vi[a * P + c] != 0.0)) {
                             val[2 * e] = vr[a * P + c]; val[2 * e + 1] = vi[a * P + c];
-                            sparse_desc(M, k, s, q, l, desc + 4 * e, more + e); ++e;
+                            if (rt) sparse_desc(M, k, s, q, l, desc + 4 * e, nullptr, rows32 + 32 * (size_t)e);
+                            else sparse_desc(M, k, s, q, l, desc + 4 * e, more + e, nullptr);
+                            ++e;
                         }
             }
     }
@@ -227,7 +319,7 @@ static int sparse_pack(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, int*
 bool mcb_sparse_preferred(mcb_space* sp, const mcb_c128* T, const mcb_c128* V)
 {
     int n1, n2; size_t bytes;
-    if (sp->M > MCB_MAX_M_TILED) return false;
+    if (sp->M > MCB_MAX_M_TILED && sp->N < 2) return false;             // (one particle, many orbitals: the M x M mat-vec needs no table)
     if (sparse_pack(sp, T, V, &n1, &n2, &bytes, true) < 0) return false;
     return 4 * (long long)n2 <= (long long)sp->P * sp->P;             // the M (M - 1) one-body entries never dominate
 }
@@ -279,8 +371,37 @@ static int launch_sparse_m(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, 
     return MCB_OK;
 }
 
+static int launch_sparse_rt(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, const mcb_c128* d_C, mcb_c128* d_HC, cudaStream_t st)
+{
+    int n1, n2; size_t bytes;
+    if (mcb_coef_stale(sp)) {
+        if (sparse_pack(sp, T, V, &n1, &n2, &bytes, false) < 0) return MCB_EUNSUPPORTED;
+        { int rc = mcb_coef_upload(sp, sp->h_coef, bytes, st); if (rc) return rc; }
+        sp->hold_n1 = n1; sp->hold_n2 = n2; sp->hold_bytes = bytes;
+        mcb_coef_staged(sp);
+    } else { n1 = sp->hold_n1; n2 = sp->hold_n2; bytes = sp->hold_bytes; }
+    SparseArgs a;
+    a.d = sp->dev; a.fock = sp->fock; a.C = (const double2*)d_C; a.HC = (double2*)d_HC;
+    a.coef = (const double2*)sp->d_coef; a.n1 = n1; a.n2 = n2;
+    a.g0 = 0; a.g1 = (int)sp->nc;
+    const size_t smem = bytes + sparse_rt_per_cta(sp->M);
+    if (smem > 227 * 1024) return MCB_EUNSUPPORTED;
+    if (smem > sp->sparse_smem_set) {
+        MCB_CUDA(cudaFuncSetAttribute(k_hc_sparse_rt, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        sp->sparse_smem_set = smem;
+    }
+    { int rc = mcb_tick(sp, 0, st); if (rc) return rc; }
+    k_hc_sparse_rt<<<(unsigned)((sp->nc + SPARSE_RT_THREADS - 1) / SPARSE_RT_THREADS), SPARSE_RT_THREADS, smem, st>>>(a);
+    MCB_CHECK_LAUNCH();
+    { int rc = mcb_tick(sp, 1, st); if (rc) return rc; }
+    mcb_tick_done(sp, 1);
+    sp->last_launches = 1;
+    return MCB_OK;
+}
+
 int mcb_launch_sparse(mcb_space* sp, const mcb_c128* T, const mcb_c128* V, const mcb_c128* d_C, mcb_c128* d_HC, cudaStream_t st)
 {
+    if (sp->M > MCB_MAX_M_TILED) return launch_sparse_rt(sp, T, V, d_C, d_HC, st);
     switch (sp->M) {
     case 1: return launch_sparse_m<1>(sp, T, V, d_C, d_HC, st);
     case 2: return launch_sparse_m<2>(sp, T, V, d_C, d_HC, st);

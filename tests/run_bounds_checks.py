@@ -68,7 +68,16 @@ def sweep():
             hC = torch.from_numpy(C).pin_memory()
             if 2 <= M <= 5:
                 assert float(np.abs(sp.hc_apply_host(T, V, hC, mode=mcb.RUNS).numpy() - ref).max()) <= t
-        sp.rho(dC)
+        if M > 12:                                                   # run-time-M MCB_SPARSE kernel: a Bose-Hubbard ring on M sites
+            Tb, Vb, _ = workloads.make_small_inputs(N, M, nc, seed=31 * N + M, kind="bh")
+            refb, _ = oracle.hc_apply(N, M, Tb, Vb, C)
+            tb = 1e-12 * max(np.abs(Tb).max(), np.abs(Vb).max()) * np.abs(C).sum()
+            for rep in range(2):
+                assert float(np.abs(sp.hc_apply(Tb, Vb, dC, mode=mcb.SPARSE).cpu().numpy() - refb).max()) <= tb
+        r1, r2 = sp.rho(dC)
+        if M <= mcb.RHO_STATIC_MAX_M:                                # the allocation-free variant: same kernels, fixed scratch
+            s1, s2 = sp.rho_static(dC)
+            assert float((s1 - r1).abs().max()) <= 1e-12 * N * max(N - 1, 1) and float((s2 - r2).abs().max()) <= 1e-12 * N * max(N - 1, 1)
         sp.lanczos(T, V, dC, min(5, nc))
         compiled, site, idx = sp.debug_bounds()
         assert compiled, "libmcb.so was not built with -DMCB_DEBUG_BOUNDS"

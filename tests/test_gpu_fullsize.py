@@ -210,15 +210,21 @@ def test_error_paths_rho_and_lanczos(mcb):
     assert e.value.status == mcb.EINVAL
     a, b = sp.lanczos(T, V, C, 5)               # H = 0: invariant subspace after one step
     assert len(a) == 1 and a[0] == 0.0 and b[0] == 0.0
-    big = mcb.Space(3, 14)                      # many orbitals: the generic path serves AUTO / GEMM only
+    big = mcb.Space(3, 14)                      # many orbitals: the generic path serves AUTO / GEMM, and SPARSE has a run-time-M kernel
     big.build_structure(mcb.FOCK_TABLE)
     Tb, Vb = np.zeros((14, 14), dtype=np.complex128), np.zeros((14,) * 4, dtype=np.complex128)
     Cb = torch.ones(big.nc, dtype=torch.complex128, device="cuda")
-    for mode in (mcb.REHASH, mcb.MAPS, mcb.RUNS, mcb.SPARSE):
+    for mode in (mcb.REHASH, mcb.MAPS, mcb.RUNS):
         with pytest.raises(mcb.McbError) as e:
             big.hc_apply(Tb, Vb, Cb, mode=mode)
         assert e.value.status == mcb.EUNSUPPORTED
-    assert big.resolve_mode(Tb, Vb) == mcb.GEMM
+    assert big.resolve_mode(Tb, Vb) == mcb.SPARSE                       # H = 0 has no off-diagonal element at all
+    assert float(big.hc_apply(Tb, Vb, Cb, mode=mcb.SPARSE).abs().max()) == 0.0
+    Vd = np.ones((14,) * 4, dtype=np.complex128)                        # a full V: the dense generic path
+    assert big.resolve_mode(Tb, Vd) == mcb.GEMM
+    with pytest.raises(mcb.McbError) as e:
+        big.hc_apply(Tb, Vd, Cb, mode=mcb.SPARSE)                       # 105 * 104 off-diagonal elements > 1024
+    assert e.value.status == mcb.EUNSUPPORTED
     sp.close()
     big.close()
 
