@@ -244,7 +244,7 @@ KERNELS = {1: ["k_hc_direct<M,maps>"], 2: ["k_hc_direct<M,rehash>"], 3: ["k_hc2_
 # captures (profiles/*.md name the commands); None where no capture of the current kernel exists.
 NCU_TRAFFIC_BYTES = {
     (2, 4): (1.437949e9 + 1.193993e9, "profiles/r2_cfg2_runs_head.md"),
-    (1, 5): (0.119567e9 + 0.047524e9, "profiles/r2_cfg1_sparse_final.md"),
+    (1, 5): (0.119572e9 + 0.048353e9, "profiles/r3_cfg1_sparse.md"),
     (4, 3): (0.452885e9 + 3.056407e9, "profiles/r2_gemm_final.md"),
     (3, 3): (0.612919e9 + 4.066090e9, "profiles/r2_gemm_final.md"),
     (2, 1): (5.121572e9 + 0.172730e9, "profiles/r2_cfg2_maps_final.md"),
